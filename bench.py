@@ -1,0 +1,323 @@
+#!/usr/bin/env python
+"""bench.py -- the hot path of arXiv 1311.2719 on B200: conjugate-gradient fermion solver.
+
+One "step" = one call of the paper's congrad: the whole hot path of SURVEY.md
+8(a) -- init (S6), then per iteration Dslash-1 + alpha (S1,S2), Dslash-2 fused with the x/r
+updates and |r|^2 (S3), the convergence scalar (S4), the p-update (S5), and the true-residual
+check (S7) -- on BASELINE.json config 3 (32^4 staggered, Haar links, m = 0.01, tol 1e-10), the
+configuration the north-star target is quoted on.  `value` = algorithmic HBM bytes of the solve
+(2832 B per site and iteration + init + final check) / time-to-solution, summed
+over ranks; `ms_per_step` is the CG time-to-solution.  `roofline` is the plain staggered Dslash
+kernel (1248 B per output site) timed with CUDA events on the library's stream.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1..5]
+
+N > 1 (torchrun): replicas only -- every rank solves its own right-hand side on the same gauge
+field, no data-path collective; scaling = weak.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_1311_2719_b200 import synth  # noqa: E402  (input generators only)
+
+STAG_DSLASH_BYTES = 1248   # per output site: 8 links x 144 B + 48 B in + 48 B out
+STAG_DSLASH_FLOPS = 570
+WILSON_DSLASH_BYTES = 1536
+WILSON_DSLASH_FLOPS = 1320
+NOMINAL_HBM_GBS = 8000.0
+FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
+
+
+def cg_bytes(cfg, iters: int) -> float:
+    """Algorithmic HBM bytes of one solve."""
+    v = synth.volume(cfg["dims"])
+    if cfg["fermion"] == "staggered":
+        vh, vec = v // 2, 48
+        per_iter = 2 * 1152 + 11 * vec                    # 2832 B / site / iteration
+        fixed = 4 * vec + (1152 + 2 * vec) + (1152 + 4 * vec)  # init + D_oe x + fused residual
+        return float(vh) * (per_iter * iters + fixed)
+    vec = 192
+    per_iter = 2 * 1152 + 11 * vec                        # two full-lattice hops + 11 vector passes
+    fixed = 4 * vec + (1152 + 2 * vec) + (1152 + 3 * vec)
+    return float(v) * (per_iter * iters + fixed)
+
+
+def hbm_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            return float(json.load(open(path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled every 200 ms during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "200"],
+                                      stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.p.terminate()
+        try:
+            out, _ = self.p.communicate(timeout=5)
+        except Exception:
+            self.p.kill()
+            out = ""
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            f = [t.strip() for t in line.split(",")]
+            if len(f) < 6:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, val in zip(names, f[2:6]):
+                if val.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_arm(cfg, u, b, steps, warmup, target_seconds=6.0):
+    """The oracle as it stands on the host cores: each step = `n_it` CG iterations (tol = 0)."""
+    import oracle
+    f = 0 if cfg["fermion"] == "staggered" else 1
+    t0 = time.perf_counter()
+    oracle.cg(cfg["dims"], f, u, cfg["param"], 0.0, 1, b)
+    t1 = time.perf_counter() - t0
+    n_it = max(1, int(target_seconds / max(t1 / 2.0, 1e-6)))   # a 1-iteration call applies A twice (loop + check)
+    n_it = min(n_it, 200)
+    for _ in range(warmup):
+        oracle.cg(cfg["dims"], f, u, cfg["param"], 0.0, 1, b)
+    times = []
+    for _ in range(steps):
+        t0 = time.perf_counter()
+        oracle.cg(cfg["dims"], f, u, cfg["param"], 0.0, n_it, b)
+        times.append(time.perf_counter() - t0)
+    sec = sum(times) / len(times)
+    return {"value": cg_bytes(cfg, n_it) / sec / 1e9, "unit": "GB/s", "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": "%d CG iterations (tol=0) of the %s solve per step, %d steps, %.2f s/step"
+                      % (n_it, cfg["name"], steps, sec), "ms_per_step": sec * 1e3, "iters_per_step": n_it}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--cg-mode", default="graph", choices=["sync", "async", "graph"])
+    ap.add_argument("--check-every", type=int, default=8)
+    ap.add_argument("--dslash-reps", type=int, default=200)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    cfg = synth.config(args.config)
+    workload = "%s: %s %s, %s links, %s=%g, tol=%g, fp64" % (
+        cfg["name"], "x".join(map(str, cfg["dims"])), cfg["fermion"], cfg["links"],
+        "mass" if cfg["fermion"] == "staggered" else "kappa", cfg["param"], cfg["tol"])
+    metric = "CG solve effective HBM throughput (algorithmic bytes of Dslash + fused updates / time-to-solution)"
+
+    # ------------------------------------------------------------------ reference arm = the oracle
+    if args.impl == "reference":
+        if rank != 0:
+            return 0
+        u = synth.gauge_field(cfg["dims"], cfg["links"], cfg["seed"])
+        b = synth.source(cfg["dims"], cfg["fermion"], cfg["seed"])
+        r = oracle_arm(cfg, u, b, max(1, args.steps), max(0, args.warmup), target_seconds=8.0)
+        line = {"impl": "reference", "metric": metric, "value": r["value"], "unit": "GB/s", "n_gpus": 0,
+                "steps": args.steps, "warmup": args.warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": workload, "sample": r["sample"]},
+                "cpu_baseline": {"value": r["value"], "unit": "GB/s", "cores": r["cores"], "kind": "oracle",
+                                 "sample": r["sample"]},
+                "e2e": {"value": r["value"], "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                "gpu_launches": 0}
+        print(json.dumps(line))
+        return 0
+
+    # ------------------------------------------------------------------ our arm
+    import torch
+    import torch.distributed as dist
+    from paper_1311_2719_b200 import lqcd
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the CUDA path is the only path")
+    torch.cuda.set_device(local_rank)
+    device = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=device)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x: float) -> float:
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def sum_over_ranks(x: float) -> float:
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        return float(t.item())
+
+    f = lqcd.STAGGERED if cfg["fermion"] == "staggered" else lqcd.WILSON
+    u = synth.gauge_field(cfg["dims"], cfg["links"], cfg["seed"])
+    b = synth.source(cfg["dims"], cfg["fermion"], cfg["seed"] + 1000 * rank)   # one right-hand side per rank
+    u_host = torch.from_numpy(u).pin_memory()
+    b_host = torch.from_numpy(b).pin_memory()
+    lat = lqcd.Lattice(cfg["dims"], f, device=device)
+    lat.set_option(lqcd.OPT_CG_MODE, {"sync": lqcd.CG_SYNC, "async": lqcd.CG_ASYNC, "graph": lqcd.CG_GRAPH}[args.cg_mode])
+    lat.set_option(lqcd.OPT_CG_CHECK_EVERY, args.check_every)
+    u_dev = u_host.to(device, non_blocking=True)
+    b_dev = b_host.to(device, non_blocking=True)
+    lat.load_gauge(u_dev)
+    x_dev = lat.new_vector()
+    maxiter = 100000
+    v = synth.volume(cfg["dims"])
+    sites_out = v // 2   # output sites of one parity Dslash
+
+    # warm-up
+    iters = res = None
+    for _ in range(max(args.warmup, 3)):
+        _, iters, res, status = lat.cg_solve(cfg["param"], cfg["tol"], maxiter, b_dev, x_dev)
+    assert status == 0, "CG did not converge"
+
+    # ---- timed region 1: K whole solves, device-resident inputs
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    launches0 = lat.kernel_launches()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(lat.stream)
+    for _ in range(args.steps):
+        _, iters, res, status = lat.cg_solve(cfg["param"], cfg["tol"], maxiter, b_dev, x_dev)
+    e1.record(lat.stream)
+    barrier()
+    ms_solve = max_over_ranks(e0.elapsed_time(e1)) / args.steps
+    launches = lat.kernel_launches() - launches0
+    total_bytes = sum_over_ranks(cg_bytes(cfg, iters))
+    value = total_bytes / (ms_solve * 1e-3) / 1e9
+
+    # ---- timed region 2: the dominant kernel alone (plain Dslash), CUDA events on its stream.
+    # Inputs (0.6 GB of links at cfg 3) exceed the 126 MB L2, parities alternate.
+    if f == lqcd.STAGGERED:
+        va, vb = lat.new_vector(), lat.new_vector()
+        va.copy_(b_dev)
+        dbytes, dflops = STAG_DSLASH_BYTES, STAG_DSLASH_FLOPS
+    else:
+        va, vb = lat.new_vector(), lat.new_vector()
+        va.copy_(b_dev)
+        vb.zero_()
+        dbytes, dflops = WILSON_DSLASH_BYTES, WILSON_DSLASH_FLOPS
+    for i in range(6):
+        lat.dslash(1 - (i & 1), va if not (i & 1) else vb, vb if not (i & 1) else va)
+    d0, d1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    d0.record(lat.stream)
+    for i in range(args.dslash_reps):
+        lat.dslash(1 - (i & 1), va if not (i & 1) else vb, vb if not (i & 1) else va)
+    d1.record(lat.stream)
+    barrier()
+    us_dslash = max_over_ranks(d0.elapsed_time(d1)) * 1e3 / args.dslash_reps
+    clocks = sampler.stop() if sampler else None
+    peak, peak_src = hbm_peak()
+    achieved = dbytes * sites_out / (us_dslash * 1e-6) / 1e9
+
+    # ---- e2e: the paper's congrad with its data region, HOST buffers through the C-ABI
+    e2e = None
+    if not args.no_e2e:
+        x_host = torch.empty(lat.vector_shape, dtype=torch.complex128).pin_memory()
+        lat.congrad_host(u_host, cfg["param"], cfg["tol"], maxiter, b_host, x_host)   # warm
+        n_e2e = max(1, min(args.steps, 3))
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            _, it_e, res_e, st_e = lat.congrad_host(u_host, cfg["param"], cfg["tol"], maxiter, b_host, x_host)
+        torch.cuda.synchronize()
+        sec = max_over_ranks(time.perf_counter() - t0) / n_e2e
+        e2e = {"value": sum_over_ranks(cg_bytes(cfg, it_e)) / sec / 1e9, "unit": "GB/s", "ms_per_step": sec * 1e3,
+               "h2d_bytes_per_step": int(u_host.numel() * 16 + b_host.numel() * 16),
+               "d2h_bytes_per_step": int(x_host.numel() * 16 + 96), "iters": it_e, "true_residual": res_e,
+               "api": "lqcd_congrad_host (pinned host u, b -> x)"}
+
+    # ---- the oracle beside it (rank 0, N = 1 only)
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        r = oracle_arm(cfg, u, b, steps=2, warmup=0, target_seconds=6.0)
+        cpu = {"value": r["value"], "unit": "GB/s", "cores": r["cores"], "kind": "oracle", "sample": r["sample"]}
+
+    if rank == 0:
+        line = {
+            "metric": metric, "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_solve, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload, "cg_mode": args.cg_mode, "check_every": args.check_every,
+                       "parallelism": "replicas x%d (independent right-hand sides)" % world,
+                       "l2_policy": "inputs larger than L2 (%.0f MB of links per Dslash), no flush" % (v * 576 / 1e6)},
+            "cg": {"time_to_solution_ms": ms_solve, "iters": iters, "true_residual": res,
+                   "us_per_iteration": ms_solve * 1e3 / max(iters, 1)},
+            "dslash": {"us_per_call": us_dslash, "GBps": achieved, "GFLOPs": dflops * sites_out / (us_dslash * 1e-6) / 1e9,
+                       "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS, "reps": args.dslash_reps},
+            "roofline": {"bound": "hbm", "kernel": "stag_dslash_kernel<SE_PLAIN>" if f == lqcd.STAGGERED else
+                         "wilson_dslash_kernel<WE_PLAIN>", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                         "frac": achieved / peak, "peak_source": peak_src, "traffic": None,
+                         "bytes_per_site": dbytes, "sites_per_launch": sites_out},
+            "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "cpu_baseline": cpu,
+        }
+        prof = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(prof):   # per-launch DRAM bytes of the same kernel from the committed ncu capture
+            try:
+                t = json.load(open(prof)).get("%s_dslash_plain" % cfg["name"])
+                if t:
+                    line["roofline"]["traffic"] = t
+            except Exception:
+                pass
+        print(json.dumps(line))
+    lat.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

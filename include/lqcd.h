@@ -1,0 +1,145 @@
+/*
+ * lqcd.h -- C-ABI boundary of the B200-native conjugate-gradient fermion solver of
+ * arXiv 1311.2719 ("Lattice Simulations using OpenACC compilers").
+ *
+ * The calls are those BASELINE.json `north_star` (a) lists and SURVEY.md 8(b) shapes
+ * after the paper's `congrad(nitcg)`, `fmv(offset,len,out,in)`
+ * and `fmtv(out,in)`.  Plain pointers and sizes only; no
+ * exception crosses this boundary.  Every step runs in hand-written sm_100a kernels;
+ * there is no CPU fallback: without a CUDA device every compute call returns
+ * LQCD_ECUDA.
+ *
+ * Pointer suffixes: *_dev = device memory, *_host = host memory.  The caller
+ * (PyTorch in the Python binding) allocates every device buffer and owns the CUDA
+ * stream; the library keeps no user pointer past a call except the workspace, in
+ * which it places its internal gauge copy, the CG vectors, the reduction scratch and
+ * the staging buffers of the *_host entry points.  All calls enqueue on the one
+ * stream given to lqcd_set_workspace; calls that return values to the host
+ * (get_tables, cg_solve, *_host) synchronise that stream before returning.
+ *
+ * Canonical layouts (little-endian fp64, complex = (re,im) adjacent; V = L0*L1*L2*L3,
+ * Vh = V/2; direction mu = 0,1,2,3 <-> x,y,z,t; time is mu = 3):
+ *   site index  g = parity*Vh + e,  e = floor(s/2),  s = x0 + L0*(x1 + L1*(x2 + L2*x3)),
+ *               parity = (x0+x1+x2+x3) mod 2   (even block first, the paper's l = 1..mvd2,
+ *               PAPER.md:69, :83)
+ *   gauge       u[g][mu][row][col]    9 complex per link, U_mu(x) stored at the site it leaves
+ *   staggered   v[c][e]               c = 0..2, one parity (the paper's p(l,ic))
+ *   Wilson      v[spin][c][g]         spin = 0..3, full lattice
+ *   tables      iup[mu][g], idn[mu][g] = g-index of x+mu^, x-mu^ (periodic wrap; signs are
+ *               not in the tables);  lex2eo[s] = g
+ *
+ * Operators (the paper's section-3 listing is missing from
+ * PAPER.md:46-48):
+ *   staggered  (D chi)(x) = 1/2 sum_mu eta_mu(x) [ b+ U_mu(x) chi(x+mu^) - b- U_mu(x-mu^)^+ chi(x-mu^) ],
+ *              eta_0 = 1, eta_1 = (-1)^x0, eta_2 = (-1)^(x0+x1), eta_3 = (-1)^(x0+x1+x2);
+ *              b+- = -1 on hops across x3 = L3-1 <-> 0 (antiperiodic time), else +1.
+ *              A = (M^+ M)_ee = m^2 - D_eo D_oe on even-site vectors.
+ *   Wilson     (D_W psi)(x) = sum_mu [ (1-gamma_mu) b+ U_mu(x) psi(x+mu^) + (1+gamma_mu) b- U_mu(x-mu^)^+ psi(x-mu^) ],
+ *              DeGrand-Rossi gamma matrices, M = 1 - kappa D_W, A = M^+ M = gamma5 M gamma5 M, full lattice.
+ *
+ * Return codes: 0 = ok; LQCD_MAXITER (=1) only from the CG calls (outputs still valid);
+ * negative = error, message available from lqcd_last_error().
+ */
+#ifndef LQCD_H
+#define LQCD_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lqcd_ctx lqcd_ctx; /* opaque; owns no user memory */
+
+enum { LQCD_STAGGERED = 0, LQCD_WILSON = 1 };
+enum { LQCD_EVEN = 0, LQCD_ODD = 1 };
+enum {
+    LQCD_OK = 0,
+    LQCD_MAXITER = 1, /* CG stopped at maxiter; x, iters, true_residual are valid */
+    LQCD_EDIM = -1,   /* an extent is odd or < 2, or the volume overflows the index type */
+    LQCD_EARG = -2,   /* null pointer, bad enum, bad parity, tol < 0, maxiter < 0 */
+    LQCD_ESTATE = -3, /* workspace not set or gauge field not loaded */
+    LQCD_ECUDA = -4,  /* a CUDA call failed (including: no device) */
+    LQCD_ENOMEM = -5  /* workspace too small */
+};
+
+/* Solver variants of lqcd_set_option(LQCD_OPT_CG_MODE): all run the same arithmetic in the
+ * same order and give bit-identical iterates; they differ only in how the host learns of
+ * convergence ("update host(betan)"). */
+enum {
+    LQCD_CG_SYNC = 0,  /* the paper's scheme: one 8-byte D2H + host test per iteration */
+    LQCD_CG_ASYNC = 1, /* kernels of later iterations are enqueued while the scalar is in flight;
+                          a device-side flag turns iterations after convergence into no-ops */
+    LQCD_CG_GRAPH = 2  /* ASYNC with each batch of iterations replayed from one CUDA graph */
+};
+enum { LQCD_OPT_CG_MODE = 0, LQCD_OPT_CG_CHECK_EVERY = 1 };
+
+/* Create a context for an L0 x L1 x L2 x L3 lattice (every extent even and >= 2; L = 2 is
+ * legal: forward and backward neighbour coincide).  Host-only; touches no device. */
+int lqcd_create(lqcd_ctx **out, int L0, int L1, int L2, int L3, int fermion_type);
+int lqcd_destroy(lqcd_ctx *ctx);
+
+/* Bytes of device scratch the caller must provide (256-byte aligned), and the hand-over.
+ * `cuda_stream` is a cudaStream_t (NULL = the legacy default stream).  The workspace must
+ * outlive the context or be replaced by another lqcd_set_workspace call. */
+size_t lqcd_workspace_bytes(const lqcd_ctx *ctx);
+int lqcd_set_workspace(lqcd_ctx *ctx, void *workspace_dev, size_t bytes, void *cuda_stream);
+
+/* Integer options (above).  Returns LQCD_EARG for an unknown option or value. */
+int lqcd_set_option(lqcd_ctx *ctx, int option, int value);
+
+/* Convert the canonical gauge field u_dev[V][4][3][3] (complex) into the library's
+ * structure-of-arrays copy inside the workspace (the paper's
+ * copyin(u) + linkc_acc).  u_dev is not referenced after the call returns
+ * control to the stream (stream-ordered). */
+int lqcd_load_gauge(lqcd_ctx *ctx, const double *u_dev);
+
+/* Neighbour and index tables (the paper's iup, idn), built on the device
+ * by the same index arithmetic the Dslash kernels use and copied to host arrays
+ * iup_host[4][V], idn_host[4][V], lex2eo_host[V].  Any of the three may be NULL. */
+int lqcd_get_tables(lqcd_ctx *ctx, int32_t *iup_host, int32_t *idn_host, int32_t *lex2eo_host);
+
+/* Bare hopping term, no mass / kappa (the paper's fmv / fmtv).
+ * Staggered: in_dev[3][Vh] lives on parity 1-out_parity, out_dev[3][Vh] on out_parity.
+ * Wilson: in_dev and out_dev are full-lattice vectors [4][3][V]; the half of in_dev on parity
+ * 1-out_parity is read and only the out_parity half of out_dev is written.
+ * in_dev and out_dev must not alias. */
+int lqcd_dslash(lqcd_ctx *ctx, int out_parity, const double *in_dev, double *out_dev);
+
+/* out = A in.  Staggered: even-site vectors, A = mass^2 - D_eo D_oe.  Wilson: full-lattice
+ * vectors, A = gamma5 M gamma5 M with M = 1 - kappa D_W.  No aliasing. */
+int lqcd_apply_MdagM(lqcd_ctx *ctx, double mass_or_kappa, const double *in_dev, double *out_dev);
+
+/* Conjugate gradient on A x = b from x = 0 (the paper's congrad; steps
+ * S1-S7 of SURVEY.md 8(a)): stops when <r,r> <= tol^2 <b,b> (tol = 0: run exactly maxiter
+ * iterations) or after maxiter iterations (returns LQCD_MAXITER).  *iters = number of
+ * applications of A inside the loop; *true_residual = |b - A x| / |b| from a fresh A.
+ * b = 0 gives x = 0, iters = 0, true_residual = 0.  b_dev and x_dev must not alias. */
+int lqcd_cg_solve(lqcd_ctx *ctx, double mass_or_kappa, double tol, int maxiter, const double *b_dev, double *x_dev,
+                  int *iters, double *true_residual);
+
+/* The paper's congrad with its data region (copyin(u,r) ... copyout(x)):
+ * HOST buffers in the canonical layouts (pinned memory makes the copies asynchronous).
+ * Copies u and b to the device, converts the gauge field, solves, copies x back. */
+int lqcd_congrad_host(lqcd_ctx *ctx, const double *u_host, double mass_or_kappa, double tol, int maxiter,
+                      const double *b_host, double *x_host, int *iters, double *true_residual);
+
+/* Host-buffer form of lqcd_dslash (copies in_host up, out_host down; gauge must be loaded). */
+int lqcd_dslash_host(lqcd_ctx *ctx, int out_parity, const double *in_host, double *out_host);
+
+/* Residual history of the last CG call: <r,r> after iteration k at index k (index 0 = <b,b>),
+ * for k <= min(iters, 65535).  Copies at most `capacity` values to rr_host and returns the
+ * number copied (negative = error). */
+int lqcd_cg_history(lqcd_ctx *ctx, double *rr_host, int capacity);
+
+/* Number of kernels launched by this context since creation (for bench.py's gpu_launches). */
+long long lqcd_kernel_launches(const lqcd_ctx *ctx);
+
+/* Text of the last error on this context ("" if none).  Valid until the next call on ctx. */
+const char *lqcd_last_error(const lqcd_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LQCD_H */

@@ -1,0 +1,109 @@
+// cg_kernels.cuh -- the CG vector kernels, the one-off gauge
+// reordering (S0) and the neighbour-table builder.
+#pragma once
+#include "reduce.cuh"
+
+namespace lqcd {
+
+// S6: p = r = b, x = 0, betan = <r,r> in one pass; also bb, pp and the CG
+// bookkeeping.  n = number of complex elements of a CG vector.
+template <int BLOCK>
+__global__ void __launch_bounds__(BLOCK) cg_init_kernel(const cplx* __restrict__ b, cplx* __restrict__ x,
+                                                        cplx* __restrict__ r, cplx* __restrict__ p, size_t n,
+                                                        CgScalars* sc, ReduceScratch rs, double* hist, double tol,
+                                                        int maxiter)
+{
+    double local = 0.0;
+    for (size_t i = (size_t)blockIdx.x * BLOCK + threadIdx.x; i < n; i += (size_t)gridDim.x * BLOCK) {
+        const cplx v = b[i];
+        r[i] = v;
+        p[i] = v;
+        x[i] = cmake(0.0, 0.0);
+        local += cnorm2(v);
+    }
+    grid_sum<BLOCK>(local, rs, [sc, hist, tol, maxiter](double bb) {
+        sc->rr = bb;
+        sc->rr_new = bb;
+        sc->bb = bb;
+        sc->pp = bb;
+        sc->tt = 0.0;
+        sc->alpha = 0.0;
+        sc->beta = 0.0;
+        sc->thresh = tol * tol * bb;
+        sc->res2 = 0.0;
+        sc->iter = 0;
+        sc->maxiter = maxiter;
+        sc->done = (bb == 0.0 || maxiter <= 0) ? 1 : 0;  // b = 0: x = 0, iters = 0 (reading A11)
+        hist[0] = bb;
+    });
+}
+
+// S5 (PAPER.md:96 gives beta; the p-update itself fell off the truncated listing, reading A7):
+// p = r + beta p, pp = <p,p>.
+template <int BLOCK>
+__global__ void __launch_bounds__(BLOCK) cg_pupdate_kernel(const cplx* __restrict__ r, cplx* __restrict__ p, size_t n,
+                                                           CgScalars* sc, ReduceScratch rs)
+{
+    if (sc->done) return;
+    const double beta = sc->beta;
+    double local = 0.0;
+    for (size_t i = (size_t)blockIdx.x * BLOCK + threadIdx.x; i < n; i += (size_t)gridDim.x * BLOCK) {
+        const cplx rv = r[i];
+        cplx pv = p[i];
+        pv.x = fma(beta, pv.x, rv.x);
+        pv.y = fma(beta, pv.y, rv.y);
+        p[i] = pv;
+        local += cnorm2(pv);
+    }
+    grid_sum<BLOCK>(local, rs, [sc](double pp) { sc->pp = pp; });
+}
+
+// S0: canonical u[g][mu][3][3] (array of structures, 576 B per site) -> [parity][mu][9][Vh]
+// (structure of arrays).  A block stages TILE sites through shared memory so both the global
+// read and the global write are contiguous.
+template <int BLOCK, int TILE>
+__global__ void __launch_bounds__(BLOCK) gauge_reorder_kernel(const cplx* __restrict__ u, cplx* __restrict__ soa,
+                                                              size_t Vh)
+{
+    __shared__ cplx tile[TILE * 36 + 1];
+    const size_t V = 2 * Vh;
+    const size_t g0 = (size_t)blockIdx.x * TILE;
+    const size_t nsite = g0 + TILE <= V ? TILE : V - g0;
+    for (size_t i = threadIdx.x; i < nsite * 36; i += BLOCK) tile[i] = u[g0 * 36 + i];
+    __syncthreads();
+    for (size_t i = threadIdx.x; i < nsite * 36; i += BLOCK) {
+        const size_t j = i / nsite;  // mu*9 + k
+        const size_t s = i - j * nsite;
+        const size_t g = g0 + s;
+        const size_t parity = g >= Vh ? 1 : 0;
+        const size_t e = g - parity * Vh;
+        soa[(parity * 36 + j) * Vh + e] = tile[s * 36 + j];
+    }
+}
+
+// The paper's iup / idn as g-indices, from the same nbr_fwd / nbr_bwd the
+// Dslash kernels use, plus lex2eo[s] = g.
+__global__ void tables_kernel(Geom g, int32_t* __restrict__ iup, int32_t* __restrict__ idn,
+                              int32_t* __restrict__ lex2eo)
+{
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= g.V) return;
+    const int parity = idx >= g.Vh ? 1 : 0;
+    const int e = (int)(idx - (long long)parity * g.Vh);
+    const Site s = decode_site(g, parity, e);
+    const long long other = (long long)(1 - parity) * g.Vh;
+    iup[0 * g.V + idx] = (int32_t)(other + nbr_fwd<0>(g, s));
+    iup[1 * g.V + idx] = (int32_t)(other + nbr_fwd<1>(g, s));
+    iup[2 * g.V + idx] = (int32_t)(other + nbr_fwd<2>(g, s));
+    iup[3 * g.V + idx] = (int32_t)(other + nbr_fwd<3>(g, s));
+    idn[0 * g.V + idx] = (int32_t)(other + nbr_bwd<0>(g, s));
+    idn[1 * g.V + idx] = (int32_t)(other + nbr_bwd<1>(g, s));
+    idn[2 * g.V + idx] = (int32_t)(other + nbr_bwd<2>(g, s));
+    idn[3 * g.V + idx] = (int32_t)(other + nbr_bwd<3>(g, s));
+    const long long L0 = 2LL * g.Lh;
+    const long long x0 = 2LL * s.xh + s.r;
+    const long long lex = x0 + L0 * (s.x1 + (long long)g.L1 * (s.x2 + (long long)g.L2 * s.x3));
+    lex2eo[lex] = (int32_t)idx;
+}
+
+}  // namespace lqcd

@@ -1,0 +1,582 @@
+// lqcd_api.cu -- the C-ABI of include/lqcd.h: context, workspace carving, kernel launches and
+// the host side of the conjugate gradient (the paper's congrad).
+//
+// Build: nvcc -gencode arch=compute_100a,code=sm_100a -O3 -lineinfo -shared ... (build.py)
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include "../../include/lqcd.h"
+#include "cg_kernels.cuh"
+#include "stag_dslash.cuh"
+#include "wilson_dslash.cuh"
+
+using namespace lqcd;
+
+namespace {
+
+constexpr int kStagBlock = 128;
+constexpr int kWilsonBlock = 128;
+constexpr int kVecBlock = 256;
+constexpr int kReorderTile = 64;
+constexpr size_t kAlign = 256;
+
+size_t align_up(size_t n) { return (n + kAlign - 1) / kAlign * kAlign; }
+
+}  // namespace
+
+struct lqcd_ctx {
+    int L[4];
+    int fermion;
+    Geom g;
+    size_t nvec;  // complex numbers per CG vector
+    // workspace layout (byte offsets)
+    size_t off_gauge, off_r, off_p, off_t, off_sc, off_ticket, off_partials, off_hist, off_stage;
+    size_t off_stage_b, off_stage_x;  // inside the staging area, after the canonical gauge copy
+    size_t ws_needed;
+    size_t max_blocks;
+    // bound workspace
+    char* ws;
+    cudaStream_t stream;
+    bool gauge_loaded;
+    // options
+    int cg_mode;
+    int check_every;
+    // host side
+    CgScalars* h_sc;  // pinned, 2 slots
+    cudaEvent_t ev[2];
+    bool host_ready;
+    long long launches;
+    int last_iters;
+    char err[320];
+
+    cplx* gauge() const { return (cplx*)(ws + off_gauge); }
+    cplx* r() const { return (cplx*)(ws + off_r); }
+    cplx* p() const { return (cplx*)(ws + off_p); }
+    cplx* t() const { return (cplx*)(ws + off_t); }
+    CgScalars* sc() const { return (CgScalars*)(ws + off_sc); }
+    double* hist() const { return (double*)(ws + off_hist); }
+    ReduceScratch rs() const
+    {
+        ReduceScratch s;
+        s.partials = (double*)(ws + off_partials);
+        s.ticket = (unsigned int*)(ws + off_ticket);
+        return s;
+    }
+};
+
+namespace {
+
+int fail(lqcd_ctx* c, int code, const char* fmt, ...)
+{
+    if (c) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(c->err, sizeof c->err, fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+#define LQCD_CUDA(call)                                                                                  \
+    do {                                                                                                 \
+        cudaError_t e_ = (call);                                                                         \
+        if (e_ != cudaSuccess)                                                                           \
+            return fail(ctx, LQCD_ECUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, \
+                        __LINE__);                                                                       \
+    } while (0)
+
+#define LQCD_LAUNCH_CHECK()                                                                              \
+    do {                                                                                                 \
+        ctx->launches++;                                                                                 \
+        cudaError_t e_ = cudaGetLastError();                                                             \
+        if (e_ != cudaSuccess)                                                                           \
+            return fail(ctx, LQCD_ECUDA, "kernel launch failed: %s (%s:%d)", cudaGetErrorString(e_),     \
+                        __FILE__, __LINE__);                                                             \
+    } while (0)
+
+int check_ready(lqcd_ctx* ctx, bool need_gauge)
+{
+    if (!ctx) return LQCD_EARG;
+    if (!ctx->ws) return fail(ctx, LQCD_ESTATE, "workspace not set (call lqcd_set_workspace)");
+    if (need_gauge && !ctx->gauge_loaded) return fail(ctx, LQCD_ESTATE, "gauge field not loaded (call lqcd_load_gauge)");
+    return LQCD_OK;
+}
+
+unsigned int blocks_for(size_t n, int block) { return (unsigned int)((n + block - 1) / block); }
+
+unsigned int vec_grid(const lqcd_ctx* ctx)
+{
+    size_t b = (ctx->nvec + kVecBlock - 1) / kVecBlock;
+    const size_t cap = 148 * 8;
+    if (b > cap) b = cap;
+    if (b < 1) b = 1;
+    return (unsigned int)b;
+}
+
+// ---------------------------------------------------------------- staggered launches
+StagArgs stag_args(const lqcd_ctx* ctx, int parity, const cplx* in, cplx* out)
+{
+    StagArgs a;
+    memset(&a, 0, sizeof a);
+    a.g = ctx->g;
+    a.parity = parity;
+    a.gauge = ctx->gauge();
+    a.in = in;
+    a.out = out;
+    a.sc = ctx->sc();
+    a.rs = ctx->rs();
+    a.hist = ctx->hist();
+    return a;
+}
+
+template <int EPI>
+int launch_stag(lqcd_ctx* ctx, const StagArgs& a)
+{
+    stag_dslash_kernel<EPI, kStagBlock><<<blocks_for(ctx->g.Vh, kStagBlock), kStagBlock, 0, ctx->stream>>>(a);
+    LQCD_LAUNCH_CHECK();
+    return LQCD_OK;
+}
+
+// ---------------------------------------------------------------- Wilson launches
+WilsonArgs wilson_args(const lqcd_ctx* ctx, int parity, const cplx* in, cplx* out, double kappa)
+{
+    WilsonArgs a;
+    memset(&a, 0, sizeof a);
+    a.g = ctx->g;
+    a.parity = parity;
+    a.gauge = ctx->gauge();
+    a.in = in;
+    a.out = out;
+    a.kappa = kappa;
+    a.sc = ctx->sc();
+    a.rs = ctx->rs();
+    a.hist = ctx->hist();
+    return a;
+}
+
+template <int EPI, bool DAGGER>
+int launch_wilson(lqcd_ctx* ctx, const WilsonArgs& a)
+{
+    const size_t n = EPI == WE_PLAIN ? (size_t)ctx->g.Vh : (size_t)ctx->g.V;
+    wilson_dslash_kernel<EPI, DAGGER, kWilsonBlock><<<blocks_for(n, kWilsonBlock), kWilsonBlock, 0, ctx->stream>>>(a);
+    LQCD_LAUNCH_CHECK();
+    return LQCD_OK;
+}
+
+// ---------------------------------------------------------------- operator pieces
+// t = "first half" of A applied to v (D_oe v  or  M v), optionally with the norm/alpha epilogue.
+int op_first(lqcd_ctx* ctx, double param, const cplx* v, bool with_norm)
+{
+    if (ctx->fermion == LQCD_STAGGERED) {
+        StagArgs a = stag_args(ctx, LQCD_ODD, v, ctx->t());
+        a.m2 = param * param;
+        return with_norm ? launch_stag<SE_NORM>(ctx, a) : launch_stag<SE_PLAIN>(ctx, a);
+    }
+    WilsonArgs a = wilson_args(ctx, 0, v, ctx->t(), param);
+    return with_norm ? launch_wilson<WE_M_NORM, false>(ctx, a) : launch_wilson<WE_M, false>(ctx, a);
+}
+
+int cg_iteration_kernels(lqcd_ctx* ctx, double param, cplx* x)
+{
+    int rc = op_first(ctx, param, ctx->p(), true);  // S1 + S2
+    if (rc) return rc;
+    if (ctx->fermion == LQCD_STAGGERED) {           // S3
+        StagArgs a = stag_args(ctx, LQCD_EVEN, ctx->t(), nullptr);
+        a.m2 = param * param;
+        a.p = ctx->p();
+        a.x = x;
+        a.r = ctx->r();
+        return launch_stag<SE_CGUPDATE>(ctx, a);
+    }
+    WilsonArgs a = wilson_args(ctx, 0, ctx->t(), nullptr, param);
+    a.p = ctx->p();
+    a.x = x;
+    a.r = ctx->r();
+    return launch_wilson<WE_CGUPDATE, true>(ctx, a);
+}
+
+int cg_pupdate(lqcd_ctx* ctx)  // S5
+{
+    cg_pupdate_kernel<kVecBlock><<<vec_grid(ctx), kVecBlock, 0, ctx->stream>>>(ctx->r(), ctx->p(), ctx->nvec, ctx->sc(),
+                                                                              ctx->rs());
+    LQCD_LAUNCH_CHECK();
+    return LQCD_OK;
+}
+
+int enqueue_batch(lqcd_ctx* ctx, double param, cplx* x, int batch)
+{
+    for (int k = 0; k < batch; ++k) {
+        int rc = cg_iteration_kernels(ctx, param, x);
+        if (rc) return rc;
+        rc = cg_pupdate(ctx);
+        if (rc) return rc;
+    }
+    return LQCD_OK;
+}
+
+struct GraphHolder {
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    ~GraphHolder()
+    {
+        if (exec) cudaGraphExecDestroy(exec);
+        if (graph) cudaGraphDestroy(graph);
+    }
+};
+
+int read_scalars(lqcd_ctx* ctx, int slot)
+{
+    LQCD_CUDA(cudaMemcpyAsync(&ctx->h_sc[slot], ctx->sc(), sizeof(CgScalars), cudaMemcpyDeviceToHost, ctx->stream));
+    LQCD_CUDA(cudaEventRecord(ctx->ev[slot], ctx->stream));
+    return LQCD_OK;
+}
+
+int ensure_host(lqcd_ctx* ctx)
+{
+    if (ctx->host_ready) return LQCD_OK;
+    LQCD_CUDA(cudaHostAlloc((void**)&ctx->h_sc, 2 * sizeof(CgScalars), cudaHostAllocDefault));
+    LQCD_CUDA(cudaEventCreateWithFlags(&ctx->ev[0], cudaEventDisableTiming));
+    LQCD_CUDA(cudaEventCreateWithFlags(&ctx->ev[1], cudaEventDisableTiming));
+    ctx->host_ready = true;
+    return LQCD_OK;
+}
+
+}  // namespace
+
+// =========================================================================== C-ABI
+extern "C" {
+
+int lqcd_create(lqcd_ctx** out, int L0, int L1, int L2, int L3, int fermion_type)
+{
+    if (!out) return LQCD_EARG;
+    *out = nullptr;
+    if (fermion_type != LQCD_STAGGERED && fermion_type != LQCD_WILSON) return LQCD_EARG;
+    const int L[4] = { L0, L1, L2, L3 };
+    long long V = 1;
+    for (int mu = 0; mu < 4; ++mu) {
+        if (L[mu] < 2 || (L[mu] & 1)) return LQCD_EDIM;
+        V *= L[mu];
+        if (V > (1LL << 30)) return LQCD_EDIM;  // int32 tables and 32-bit half-lattice indices
+    }
+    lqcd_ctx* c = (lqcd_ctx*)calloc(1, sizeof(lqcd_ctx));
+    if (!c) return LQCD_ENOMEM;
+    memcpy(c->L, L, sizeof L);
+    c->fermion = fermion_type;
+    c->g.Lh = L0 / 2;
+    c->g.L1 = L1;
+    c->g.L2 = L2;
+    c->g.L3 = L3;
+    c->g.s1 = c->g.Lh;
+    c->g.s2 = c->g.Lh * L1;
+    c->g.s3 = c->g.Lh * L1 * L2;
+    c->g.V = V;
+    c->g.Vh = (int)(V / 2);
+    c->nvec = fermion_type == LQCD_STAGGERED ? 3 * (size_t)(V / 2) : 12 * (size_t)V;
+    c->max_blocks = (size_t)V / 64 + 4096;
+    c->cg_mode = LQCD_CG_ASYNC;
+    c->check_every = 4;
+
+    size_t off = 0;
+    const size_t vec_bytes = align_up(c->nvec * sizeof(cplx));
+    c->off_gauge = off;      off += align_up((size_t)V * 36 * sizeof(cplx));
+    c->off_r = off;          off += vec_bytes;
+    c->off_p = off;          off += vec_bytes;
+    c->off_t = off;          off += vec_bytes;
+    c->off_sc = off;         off += align_up(sizeof(CgScalars));
+    c->off_ticket = off;     off += kAlign;
+    c->off_partials = off;   off += align_up(c->max_blocks * sizeof(double));
+    c->off_hist = off;       off += align_up((size_t)kHistCap * sizeof(double));
+    c->off_stage = off;
+    const size_t stage_u = align_up((size_t)V * 36 * sizeof(cplx));
+    c->off_stage_b = off + stage_u;
+    c->off_stage_x = c->off_stage_b + vec_bytes;
+    size_t stage = stage_u + 2 * vec_bytes;
+    const size_t tables = align_up((size_t)V * 9 * sizeof(int32_t));
+    if (tables > stage) stage = tables;
+    off += stage;
+    c->ws_needed = off;
+    *out = c;
+    return LQCD_OK;
+}
+
+int lqcd_destroy(lqcd_ctx* ctx)
+{
+    if (!ctx) return LQCD_EARG;
+    if (ctx->host_ready) {
+        cudaFreeHost(ctx->h_sc);
+        cudaEventDestroy(ctx->ev[0]);
+        cudaEventDestroy(ctx->ev[1]);
+    }
+    free(ctx);
+    return LQCD_OK;
+}
+
+size_t lqcd_workspace_bytes(const lqcd_ctx* ctx) { return ctx ? ctx->ws_needed : 0; }
+
+int lqcd_set_workspace(lqcd_ctx* ctx, void* workspace_dev, size_t bytes, void* cuda_stream)
+{
+    if (!ctx) return LQCD_EARG;
+    if (!workspace_dev) return fail(ctx, LQCD_EARG, "workspace pointer is null");
+    if (((uintptr_t)workspace_dev) % kAlign) return fail(ctx, LQCD_EARG, "workspace must be 256-byte aligned");
+    if (bytes < ctx->ws_needed)
+        return fail(ctx, LQCD_ENOMEM, "workspace too small: %zu bytes given, %zu needed", bytes, ctx->ws_needed);
+    int ndev = 0;
+    LQCD_CUDA(cudaGetDeviceCount(&ndev));
+    if (ndev < 1) return fail(ctx, LQCD_ECUDA, "no CUDA device");
+    int rc = ensure_host(ctx);
+    if (rc) return rc;
+    ctx->ws = (char*)workspace_dev;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    ctx->gauge_loaded = false;
+    LQCD_CUDA(cudaMemsetAsync(ctx->ws + ctx->off_sc, 0, align_up(sizeof(CgScalars)) + kAlign, ctx->stream));
+    return LQCD_OK;
+}
+
+int lqcd_set_option(lqcd_ctx* ctx, int option, int value)
+{
+    if (!ctx) return LQCD_EARG;
+    if (option == LQCD_OPT_CG_MODE) {
+        if (value < LQCD_CG_SYNC || value > LQCD_CG_GRAPH) return fail(ctx, LQCD_EARG, "bad CG mode %d", value);
+        ctx->cg_mode = value;
+        return LQCD_OK;
+    }
+    if (option == LQCD_OPT_CG_CHECK_EVERY) {
+        if (value < 1 || value > 1024) return fail(ctx, LQCD_EARG, "check_every must be in 1..1024");
+        ctx->check_every = value;
+        return LQCD_OK;
+    }
+    return fail(ctx, LQCD_EARG, "unknown option %d", option);
+}
+
+int lqcd_load_gauge(lqcd_ctx* ctx, const double* u_dev)
+{
+    int rc = check_ready(ctx, false);
+    if (rc) return rc;
+    if (!u_dev) return fail(ctx, LQCD_EARG, "u_dev is null");
+    const size_t V = (size_t)ctx->g.V;
+    gauge_reorder_kernel<256, kReorderTile><<<blocks_for(V, kReorderTile), 256, 0, ctx->stream>>>(
+        (const cplx*)u_dev, ctx->gauge(), (size_t)ctx->g.Vh);
+    LQCD_LAUNCH_CHECK();
+    ctx->gauge_loaded = true;
+    return LQCD_OK;
+}
+
+int lqcd_get_tables(lqcd_ctx* ctx, int32_t* iup_host, int32_t* idn_host, int32_t* lex2eo_host)
+{
+    int rc = check_ready(ctx, false);
+    if (rc) return rc;
+    const size_t V = (size_t)ctx->g.V;
+    int32_t* d = (int32_t*)(ctx->ws + ctx->off_stage);
+    tables_kernel<<<blocks_for(V, 256), 256, 0, ctx->stream>>>(ctx->g, d, d + 4 * V, d + 8 * V);
+    LQCD_LAUNCH_CHECK();
+    if (iup_host) LQCD_CUDA(cudaMemcpyAsync(iup_host, d, 4 * V * sizeof(int32_t), cudaMemcpyDeviceToHost, ctx->stream));
+    if (idn_host)
+        LQCD_CUDA(cudaMemcpyAsync(idn_host, d + 4 * V, 4 * V * sizeof(int32_t), cudaMemcpyDeviceToHost, ctx->stream));
+    if (lex2eo_host)
+        LQCD_CUDA(cudaMemcpyAsync(lex2eo_host, d + 8 * V, V * sizeof(int32_t), cudaMemcpyDeviceToHost, ctx->stream));
+    LQCD_CUDA(cudaStreamSynchronize(ctx->stream));
+    return LQCD_OK;
+}
+
+int lqcd_dslash(lqcd_ctx* ctx, int out_parity, const double* in_dev, double* out_dev)
+{
+    int rc = check_ready(ctx, true);
+    if (rc) return rc;
+    if (!in_dev || !out_dev) return fail(ctx, LQCD_EARG, "null vector pointer");
+    if (in_dev == out_dev) return fail(ctx, LQCD_EARG, "in and out must not alias");
+    if (out_parity != LQCD_EVEN && out_parity != LQCD_ODD) return fail(ctx, LQCD_EARG, "bad parity %d", out_parity);
+    if (ctx->fermion == LQCD_STAGGERED) return launch_stag<SE_PLAIN>(ctx, stag_args(ctx, out_parity, (const cplx*)in_dev, (cplx*)out_dev));
+    return launch_wilson<WE_PLAIN, false>(ctx, wilson_args(ctx, out_parity, (const cplx*)in_dev, (cplx*)out_dev, 0.0));
+}
+
+int lqcd_apply_MdagM(lqcd_ctx* ctx, double mass_or_kappa, const double* in_dev, double* out_dev)
+{
+    int rc = check_ready(ctx, true);
+    if (rc) return rc;
+    if (!in_dev || !out_dev) return fail(ctx, LQCD_EARG, "null vector pointer");
+    if (in_dev == out_dev) return fail(ctx, LQCD_EARG, "in and out must not alias");
+    rc = op_first(ctx, mass_or_kappa, (const cplx*)in_dev, false);
+    if (rc) return rc;
+    if (ctx->fermion == LQCD_STAGGERED) {
+        StagArgs a = stag_args(ctx, LQCD_EVEN, ctx->t(), (cplx*)out_dev);
+        a.m2 = mass_or_kappa * mass_or_kappa;
+        a.p = (const cplx*)in_dev;
+        return launch_stag<SE_MDAGM>(ctx, a);
+    }
+    return launch_wilson<WE_M, true>(ctx, wilson_args(ctx, 0, ctx->t(), (cplx*)out_dev, mass_or_kappa));
+}
+
+int lqcd_cg_solve(lqcd_ctx* ctx, double mass_or_kappa, double tol, int maxiter, const double* b_dev, double* x_dev,
+                  int* iters, double* true_residual)
+{
+    int rc = check_ready(ctx, true);
+    if (rc) return rc;
+    if (!b_dev || !x_dev || !iters || !true_residual) return fail(ctx, LQCD_EARG, "null pointer argument");
+    if (b_dev == x_dev) return fail(ctx, LQCD_EARG, "b and x must not alias");
+    if (!(tol >= 0.0) || maxiter < 0) return fail(ctx, LQCD_EARG, "tol must be >= 0 and maxiter >= 0");
+    const cplx* b = (const cplx*)b_dev;
+    cplx* x = (cplx*)x_dev;
+
+    // S6: p = r = b, x = 0, rr = bb = pp = |b|^2
+    cg_init_kernel<kVecBlock><<<vec_grid(ctx), kVecBlock, 0, ctx->stream>>>(b, x, ctx->r(), ctx->p(), ctx->nvec, ctx->sc(),
+                                                                           ctx->rs(), ctx->hist(), tol, maxiter);
+    LQCD_LAUNCH_CHECK();
+
+    CgScalars* h = ctx->h_sc;
+    if (ctx->cg_mode == LQCD_CG_SYNC) {
+        // The paper's loop: one scalar comes back per iteration, the exit test runs on the host
+        // (PAPER.md:75-76, :91-93, :100).
+        rc = read_scalars(ctx, 0);
+        if (rc) return rc;
+        LQCD_CUDA(cudaEventSynchronize(ctx->ev[0]));
+        while (!h[0].done) {
+            rc = cg_iteration_kernels(ctx, mass_or_kappa, x);
+            if (rc) return rc;
+            rc = read_scalars(ctx, 0);
+            if (rc) return rc;
+            LQCD_CUDA(cudaEventSynchronize(ctx->ev[0]));
+            if (h[0].done) break;
+            rc = cg_pupdate(ctx);
+            if (rc) return rc;
+        }
+    } else {
+        // Same kernels, same order; batches of `check_every` iterations are enqueued while the
+        // previous batch's scalars are still on their way to the host.  Once the device sets
+        // `done`, every later kernel returns at once, so x, r and the iteration count are exactly
+        // those of the synchronous loop.
+        const int batch = ctx->check_every;
+        // LQCD_CG_GRAPH: the batch is captured once and replayed with one graph launch instead of
+        // 3*batch kernel launches (launch-bound small lattices).  The legacy default stream cannot
+        // be captured; there the batch is enqueued kernel by kernel as in LQCD_CG_ASYNC.
+        GraphHolder gh;
+        if (ctx->cg_mode == LQCD_CG_GRAPH && ctx->stream != nullptr && maxiter > 0) {
+            const long long counted = ctx->launches;
+            LQCD_CUDA(cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal));
+            rc = enqueue_batch(ctx, mass_or_kappa, x, batch);
+            cudaError_t ce = cudaStreamEndCapture(ctx->stream, &gh.graph);
+            if (rc) return rc;
+            LQCD_CUDA(ce);
+            LQCD_CUDA(cudaGraphInstantiate(&gh.exec, gh.graph, 0));
+            ctx->launches = counted;  // capturing launched nothing
+        }
+        int slot = 0;
+        bool pending[2] = { false, false };
+        bool finished = false;
+        long long enqueued = 0;
+        while (!finished) {
+            if (enqueued < (long long)maxiter) {
+                if (gh.exec) {
+                    LQCD_CUDA(cudaGraphLaunch(gh.exec, ctx->stream));
+                    ctx->launches += 3LL * batch;
+                } else {
+                    rc = enqueue_batch(ctx, mass_or_kappa, x, batch);
+                    if (rc) return rc;
+                }
+                enqueued += batch;
+            }
+            rc = read_scalars(ctx, slot);
+            if (rc) return rc;
+            pending[slot] = true;
+            const int other = slot ^ 1;
+            if (pending[other]) {
+                LQCD_CUDA(cudaEventSynchronize(ctx->ev[other]));
+                pending[other] = false;
+                if (h[other].done) finished = true;
+            }
+            slot = other;
+        }
+        // drain: the newest snapshot has the final values
+        LQCD_CUDA(cudaStreamSynchronize(ctx->stream));
+        rc = read_scalars(ctx, 0);
+        if (rc) return rc;
+        LQCD_CUDA(cudaEventSynchronize(ctx->ev[0]));
+    }
+
+    // S7: true residual |b - A x| / |b| with a fresh application of A
+    rc = op_first(ctx, mass_or_kappa, x, false);
+    if (rc) return rc;
+    if (ctx->fermion == LQCD_STAGGERED) {
+        StagArgs a = stag_args(ctx, LQCD_EVEN, ctx->t(), nullptr);
+        a.m2 = mass_or_kappa * mass_or_kappa;
+        a.p = x;
+        a.b = b;
+        rc = launch_stag<SE_RESIDUAL>(ctx, a);
+    } else {
+        WilsonArgs a = wilson_args(ctx, 0, ctx->t(), nullptr, mass_or_kappa);
+        a.b = b;
+        rc = launch_wilson<WE_RESIDUAL, true>(ctx, a);
+    }
+    if (rc) return rc;
+    rc = read_scalars(ctx, 0);
+    if (rc) return rc;
+    LQCD_CUDA(cudaEventSynchronize(ctx->ev[0]));
+
+    *iters = h[0].iter;
+    ctx->last_iters = h[0].iter;
+    *true_residual = h[0].bb > 0.0 ? sqrt(h[0].res2 / h[0].bb) : 0.0;
+    const bool converged = h[0].rr_new <= h[0].thresh;
+    return converged ? LQCD_OK : LQCD_MAXITER;
+}
+
+int lqcd_congrad_host(lqcd_ctx* ctx, const double* u_host, double mass_or_kappa, double tol, int maxiter,
+                      const double* b_host, double* x_host, int* iters, double* true_residual)
+{
+    int rc = check_ready(ctx, false);
+    if (rc) return rc;
+    if (!u_host || !b_host || !x_host) return fail(ctx, LQCD_EARG, "null host pointer");
+    const size_t V = (size_t)ctx->g.V;
+    cplx* su = (cplx*)(ctx->ws + ctx->off_stage);
+    cplx* sb = (cplx*)(ctx->ws + ctx->off_stage_b);
+    cplx* sx = (cplx*)(ctx->ws + ctx->off_stage_x);
+    // copyin(u, r)
+    LQCD_CUDA(cudaMemcpyAsync(su, u_host, V * 36 * sizeof(cplx), cudaMemcpyHostToDevice, ctx->stream));
+    LQCD_CUDA(cudaMemcpyAsync(sb, b_host, ctx->nvec * sizeof(cplx), cudaMemcpyHostToDevice, ctx->stream));
+    rc = lqcd_load_gauge(ctx, (const double*)su);
+    if (rc) return rc;
+    const int status = lqcd_cg_solve(ctx, mass_or_kappa, tol, maxiter, (const double*)sb, (double*)sx, iters, true_residual);
+    if (status < 0) return status;
+    // copyout(x)
+    LQCD_CUDA(cudaMemcpyAsync(x_host, sx, ctx->nvec * sizeof(cplx), cudaMemcpyDeviceToHost, ctx->stream));
+    LQCD_CUDA(cudaStreamSynchronize(ctx->stream));
+    return status;
+}
+
+int lqcd_dslash_host(lqcd_ctx* ctx, int out_parity, const double* in_host, double* out_host)
+{
+    int rc = check_ready(ctx, true);
+    if (rc) return rc;
+    if (!in_host || !out_host) return fail(ctx, LQCD_EARG, "null host pointer");
+    cplx* sb = (cplx*)(ctx->ws + ctx->off_stage_b);
+    cplx* sx = (cplx*)(ctx->ws + ctx->off_stage_x);
+    const size_t bytes = ctx->nvec * sizeof(cplx);
+    LQCD_CUDA(cudaMemcpyAsync(sb, in_host, bytes, cudaMemcpyHostToDevice, ctx->stream));
+    if (ctx->fermion == LQCD_WILSON) LQCD_CUDA(cudaMemsetAsync(sx, 0, bytes, ctx->stream));
+    rc = lqcd_dslash(ctx, out_parity, (const double*)sb, (double*)sx);
+    if (rc) return rc;
+    LQCD_CUDA(cudaMemcpyAsync(out_host, sx, bytes, cudaMemcpyDeviceToHost, ctx->stream));
+    LQCD_CUDA(cudaStreamSynchronize(ctx->stream));
+    return LQCD_OK;
+}
+
+int lqcd_cg_history(lqcd_ctx* ctx, double* rr_host, int capacity)
+{
+    int rc = check_ready(ctx, false);
+    if (rc) return rc;
+    if (!rr_host || capacity < 0) return fail(ctx, LQCD_EARG, "bad history buffer");
+    int n = ctx->last_iters + 1;
+    if (n > kHistCap) n = kHistCap;
+    if (n > capacity) n = capacity;
+    LQCD_CUDA(cudaMemcpyAsync(rr_host, ctx->hist(), (size_t)n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    LQCD_CUDA(cudaStreamSynchronize(ctx->stream));
+    return n;
+}
+
+long long lqcd_kernel_launches(const lqcd_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+const char* lqcd_last_error(const lqcd_ctx* ctx) { return ctx ? ctx->err : "null context"; }
+
+}  // extern "C"

@@ -1,0 +1,85 @@
+// reduce.cuh -- deterministic grid-wide sums without a host round trip.
+//
+// The paper reduces <r,r>, <ap,ap>, <p,p> with OpenACC reduction(+) clauses (PAPER.md:68-74,
+// :85, :90) and keeps alpha/beta on the device.  Here every kernel that
+// produces a vector also produces its norm: warp shuffles -> shared memory -> one partial per
+// block -> the last block to finish (ticket counter) adds the partials in a fixed order and
+// runs a small "finalise" functor that updates the CG scalars in device memory.  No floating
+// point atomics: the result does not depend on block scheduling, so iteration counts are
+// reproducible run to run.
+#pragma once
+#include "device_common.cuh"
+
+namespace lqcd {
+
+// CG scalars, device resident (the paper's alpha, betan, betad, alphan, alphad, nitcg).
+struct CgScalars {
+    double rr;        // <r,r> of the current residual (betad/alphan)
+    double rr_new;    // <r,r> after the update (betan)
+    double bb;        // <b,b>
+    double pp;        // <p,p>
+    double tt;        // <t,t>, t = D_oe p (staggered) or M p (Wilson)
+    double alpha;     // rr / <p,Ap>
+    double beta;      // rr_new / rr
+    double thresh;    // tol^2 * bb
+    double res2;      // |b - A x|^2 of the final check
+    double aux;       // scratch sum for the stand-alone norm kernel
+    int iter;         // completed iterations
+    int done;         // 1 once converged (or b = 0): later iterations become no-ops
+    int maxiter;
+    int pad;
+};
+
+struct ReduceScratch {
+    double* partials;      // one per block
+    unsigned int* ticket;  // zero between kernels
+};
+
+static constexpr int kHistCap = 65536;
+
+template <int BLOCK>
+__device__ __forceinline__ double block_sum(double v)
+{
+    __shared__ double warp_part[BLOCK / 32];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    __syncthreads();  // protect warp_part against a previous call
+    if (lane == 0) warp_part[w] = v;
+    __syncthreads();
+    double s = 0.0;
+    if (w == 0) {
+        s = lane < BLOCK / 32 ? warp_part[lane] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    }
+    return s;  // valid in warp 0
+}
+
+// Every thread of every block calls this once with its local contribution.  `fin(total)` runs in
+// thread 0 of the last block only.
+template <int BLOCK, class Finalise>
+__device__ __forceinline__ void grid_sum(double local, const ReduceScratch& rs, Finalise fin)
+{
+    __shared__ bool is_last;
+    double s = block_sum<BLOCK>(local);
+    if (threadIdx.x == 0) {
+        rs.partials[blockIdx.x] = s;
+        __threadfence();
+        unsigned int t = atomicAdd(rs.ticket, 1u);
+        is_last = (t == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (is_last) {
+        __threadfence();
+        double acc = 0.0;
+        for (unsigned int i = threadIdx.x; i < gridDim.x; i += BLOCK) acc += __ldcg(rs.partials + i);
+        double total = block_sum<BLOCK>(acc);
+        if (threadIdx.x == 0) {
+            *rs.ticket = 0u;
+            fin(total);
+        }
+    }
+}
+
+}  // namespace lqcd

@@ -1,0 +1,204 @@
+// wilson_dslash.cuh -- Wilson hopping term with fused CG epilogues.
+//
+//   (D_W psi)(x) = sum_mu [ (1-gamma_mu) b+ U_mu(x) psi(x+mu^) + (1+gamma_mu) b- U_mu(x-mu^)^+ psi(x-mu^) ]
+//   M = 1 - kappa D_W,   M^+ = gamma5 M gamma5 = 1 - kappa D_W^+,  D_W^+ = the same sum with the
+//   projector signs exchanged (gamma5 gamma_mu gamma5 = -gamma_mu).
+//
+// The paper only mentions its Wilson program; the operator is BASELINE.json
+// config 4's (DeGrand-Rossi basis).  In that basis every gamma_mu couples the upper spin pair
+// (0,1) to the lower pair (2,3) with entries among +-1, +-i:  (gamma psi)_s = i^K_s psi_{pi(s)}.
+// Hence (1 -+ gamma) psi has two independent spin components h_s = psi_s -+ i^K_s psi_pi(s),
+// s = 0,1, and its lower components are -+ conj(i^K_s) h_s at spin pi(s): only two SU(3)
+// matrix-vector products per hop instead of four.
+//
+// One thread per output site; full-lattice structure-of-arrays vectors v[spin][c][g].
+#pragma once
+#include "reduce.cuh"
+
+namespace lqcd {
+
+enum WilsonEpilogue {
+    WE_PLAIN = 0,     // out = D in on one parity                               (lqcd_dslash)
+    WE_M = 1,         // out = in - kappa D in, full lattice
+    WE_M_NORM = 2,    // the same + tt = |out|^2, alpha = rr/tt                 (S1, S2: <p,Ap> = |Mp|^2)
+    WE_CGUPDATE = 3,  // Ap = in - kappa D^+ in; x += alpha p; r -= alpha Ap; |r|^2   (S3)
+    WE_RESIDUAL = 4   // |b - (in - kappa D^+ in)|^2                            (S7)
+};
+
+struct WilsonArgs {
+    Geom g;
+    int parity;         // WE_PLAIN: output parity.  Other epilogues cover both parities.
+    const cplx* gauge;  // [2][4][9][Vh]
+    const cplx* in;     // [4][3][V]
+    cplx* out;          // [4][3][V]
+    const cplx* p;
+    cplx* x;
+    cplx* r;
+    const cplx* b;
+    double kappa;
+    CgScalars* sc;
+    ReduceScratch rs;
+    double* hist;
+};
+
+// gamma_mu in the DeGrand-Rossi basis: (gamma psi)_s = i^K psi_PI for the upper rows s = 0, 1.
+template <int MU> struct GammaDR;
+template <> struct GammaDR<0> { static constexpr int PI0 = 3, K0 = 1, PI1 = 2, K1 = 1; };  // rows (0,0,0,i), (0,0,i,0)
+template <> struct GammaDR<1> { static constexpr int PI0 = 3, K0 = 2, PI1 = 2, K1 = 0; };  // rows (0,0,0,-1), (0,0,1,0)
+template <> struct GammaDR<2> { static constexpr int PI0 = 2, K0 = 1, PI1 = 3, K1 = 3; };  // rows (0,0,i,0), (0,0,0,-i)
+template <> struct GammaDR<3> { static constexpr int PI0 = 2, K0 = 0, PI1 = 3, K1 = 0; };  // rows (0,0,1,0), (0,0,0,1)
+
+// One hop.  PLUS = false: projector (1 - gamma_mu); PLUS = true: (1 + gamma_mu).
+// ADJ = false: multiply by U (forward link at x); ADJ = true: by U^+ (link at x - mu^).
+template <int MU, bool PLUS, bool ADJ>
+__device__ __forceinline__ void wilson_hop(const cplx* __restrict__ link, size_t Vh, const cplx* __restrict__ src,
+                                           size_t V, double sign, cplx acc[4][3])
+{
+    typedef GammaDR<MU> G;
+    cplx U[9], psi[4][3];
+#pragma unroll
+    for (int k = 0; k < 9; ++k) U[k] = ld_stream(link + k * Vh);
+#pragma unroll
+    for (int s = 0; s < 4; ++s)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) psi[s][c] = ld_keep(src + (size_t)(s * 3 + c) * V);
+
+    // h_s = psi_s -+ i^K psi_pi(s)
+    constexpr int KH0 = PLUS ? G::K0 : (G::K0 + 2) & 3;
+    constexpr int KH1 = PLUS ? G::K1 : (G::K1 + 2) & 3;
+    // lower components: -+ conj(i^K) (U h)_s at spin pi(s)
+    constexpr int KL0 = PLUS ? (4 - G::K0) & 3 : (6 - G::K0) & 3;
+    constexpr int KL1 = PLUS ? (4 - G::K1) & 3 : (6 - G::K1) & 3;
+    cplx h0[3], h1[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        h0[c] = cscale(sign, cadd(psi[0][c], mul_i_pow<KH0>(psi[G::PI0][c])));
+        h1[c] = cscale(sign, cadd(psi[1][c], mul_i_pow<KH1>(psi[G::PI1][c])));
+    }
+#pragma unroll
+    for (int r = 0; r < 3; ++r) {
+        cplx u0 = cmake(0, 0), u1 = cmake(0, 0);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            if (ADJ) {
+                cfma_conj(u0, U[c * 3 + r], h0[c]);
+                cfma_conj(u1, U[c * 3 + r], h1[c]);
+            } else {
+                cfma(u0, U[r * 3 + c], h0[c]);
+                cfma(u1, U[r * 3 + c], h1[c]);
+            }
+        }
+        acc[0][r] = cadd(acc[0][r], u0);
+        acc[1][r] = cadd(acc[1][r], u1);
+        acc[G::PI0][r] = cadd(acc[G::PI0][r], mul_i_pow<KL0>(u0));
+        acc[G::PI1][r] = cadd(acc[G::PI1][r], mul_i_pow<KL1>(u1));
+    }
+}
+
+template <int MU, bool DAGGER>
+__device__ __forceinline__ void wilson_dir(const WilsonArgs& a, const Site& s, int parity, cplx acc[4][3])
+{
+    const size_t Vh = (size_t)a.g.Vh, V = (size_t)a.g.V;
+    const int ef = nbr_fwd<MU>(a.g, s);
+    const int eb = nbr_bwd<MU>(a.g, s);
+    const size_t other = (size_t)(1 - parity) * Vh;
+    const cplx* Uf = a.gauge + (size_t)((parity * 4 + MU) * 9) * Vh + s.e;
+    const cplx* Ub = a.gauge + (size_t)(((1 - parity) * 4 + MU) * 9) * Vh + eb;
+    // D: forward (1-gamma), backward (1+gamma);  D^+: forward (1+gamma), backward (1-gamma)
+    wilson_hop<MU, DAGGER, false>(Uf, Vh, a.in + other + ef, V, bc_fwd<MU>(a.g, s), acc);
+    wilson_hop<MU, !DAGGER, true>(Ub, Vh, a.in + other + eb, V, bc_bwd<MU>(a.g, s), acc);
+}
+
+template <int EPI, bool DAGGER, int BLOCK>
+__global__ void __launch_bounds__(BLOCK) wilson_dslash_kernel(const WilsonArgs a)
+{
+    if (EPI == WE_M_NORM || EPI == WE_CGUPDATE) {
+        if (a.sc->done) return;
+    }
+    const long long idx = (long long)blockIdx.x * BLOCK + threadIdx.x;
+    const size_t Vh = (size_t)a.g.Vh, V = (size_t)a.g.V;
+    bool active;
+    int parity, e;
+    if (EPI == WE_PLAIN) {
+        active = idx < (long long)Vh;
+        parity = a.parity;
+        e = (int)idx;
+    } else {
+        active = idx < (long long)V;
+        parity = idx >= (long long)Vh ? 1 : 0;
+        e = (int)(idx - (long long)parity * (long long)Vh);
+    }
+    const size_t gsite = (size_t)parity * Vh + (size_t)e;
+
+    cplx acc[4][3];
+#pragma unroll
+    for (int s = 0; s < 4; ++s)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) acc[s][c] = cmake(0, 0);
+    if (active) {
+        const Site st = decode_site(a.g, parity, e);
+        wilson_dir<0, DAGGER>(a, st, parity, acc);
+        wilson_dir<1, DAGGER>(a, st, parity, acc);
+        wilson_dir<2, DAGGER>(a, st, parity, acc);
+        wilson_dir<3, DAGGER>(a, st, parity, acc);
+    }
+
+    if (EPI == WE_PLAIN) {
+        if (active) {
+#pragma unroll
+            for (int k = 0; k < 12; ++k) st_vec(a.out + (size_t)k * V + gsite, acc[k / 3][k % 3]);
+        }
+        return;
+    }
+    // M-type: m = in(x) - kappa * acc
+    double local = 0.0;
+    const double alpha = (EPI == WE_CGUPDATE && active) ? a.sc->alpha : 0.0;
+    if (active) {
+#pragma unroll
+        for (int k = 0; k < 12; ++k) {
+            const size_t i = (size_t)k * V + gsite;
+            const cplx c0 = a.in[i];
+            const cplx m = cmake(fma(-a.kappa, acc[k / 3][k % 3].x, c0.x), fma(-a.kappa, acc[k / 3][k % 3].y, c0.y));
+            if (EPI == WE_M || EPI == WE_M_NORM) {
+                st_vec(a.out + i, m);
+                if (EPI == WE_M_NORM) local += cnorm2(m);
+            } else if (EPI == WE_CGUPDATE) {
+                const cplx pv = a.p[i];
+                cplx xv = a.x[i], rv = a.r[i];
+                xv.x = fma(alpha, pv.x, xv.x);
+                xv.y = fma(alpha, pv.y, xv.y);
+                rv.x = fma(-alpha, m.x, rv.x);
+                rv.y = fma(-alpha, m.y, rv.y);
+                a.x[i] = xv;
+                a.r[i] = rv;
+                local += cnorm2(rv);
+            } else {  // WE_RESIDUAL
+                const cplx bv = a.b[i];
+                const double re = bv.x - m.x, im = bv.y - m.y;
+                local += fma(re, re, im * im);
+            }
+        }
+    }
+    CgScalars* sc = a.sc;
+    if (EPI == WE_M_NORM) {
+        grid_sum<BLOCK>(local, a.rs, [sc](double tt) {
+            sc->tt = tt;
+            sc->alpha = sc->rr / tt;  // <p, M^+M p> = |M p|^2
+        });
+    } else if (EPI == WE_CGUPDATE) {
+        double* hist = a.hist;
+        grid_sum<BLOCK>(local, a.rs, [sc, hist](double rr_new) {
+            const int it = sc->iter + 1;
+            sc->iter = it;
+            sc->rr_new = rr_new;
+            if (it < kHistCap) hist[it] = rr_new;
+            sc->beta = rr_new / sc->rr;
+            sc->rr = rr_new;
+            if (rr_new <= sc->thresh || it >= sc->maxiter) sc->done = 1;
+        });
+    } else if (EPI == WE_RESIDUAL) {
+        grid_sum<BLOCK>(local, a.rs, [sc](double res2) { sc->res2 = res2; });
+    }
+}
+
+}  // namespace lqcd

@@ -18,3 +18,10 @@ def oracle_mod():
     import oracle
     oracle.build()
     return oracle
+
+
+@pytest.fixture(scope="session", autouse=True)
+def _built_library():
+    """The CUDA library is built in-tree (nvcc cross-compiles without a GPU)."""
+    from paper_1311_2719_b200 import build
+    build.build()
