@@ -64,6 +64,20 @@ def hbm_peak():
     return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def ncu_traffic(key):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the roofline kernel, from the committed
+    ncu --set full capture (profiles/traffic.csv); None if that kernel/workload was not captured."""
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
+    try:
+        for row in open(path).read().splitlines()[1:]:
+            f = row.split(",")
+            if f[0] == key:
+                return int(f[1]) + int(f[2])
+    except Exception:
+        pass
+    return None
+
+
 class ClockSampler:
     """nvidia-smi clocks and throttle reasons sampled every 200 ms during the timed region."""
     Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -304,14 +318,7 @@ def main():
                          "bytes_per_site": dbytes, "sites_per_launch": sites_out},
             "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "cpu_baseline": cpu,
         }
-        prof = os.path.join(ROOT, "profiles", "traffic.json")
-        if os.path.exists(prof):   # per-launch DRAM bytes of the same kernel from the committed ncu capture
-            try:
-                t = json.load(open(prof)).get("%s_dslash_plain" % cfg["name"])
-                if t:
-                    line["roofline"]["traffic"] = t
-            except Exception:
-                pass
+        line["roofline"]["traffic"] = ncu_traffic("%s_dslash_plain" % cfg["name"])
         print(json.dumps(line))
     lat.close()
     if world > 1:

@@ -1,0 +1,53 @@
+#!/usr/bin/env python
+"""Write tests/golden/oracle_cg_reference.json: what the CPU ORACLE's conjugate gradient gives on
+the BASELINE.json configs (iteration count, true residual, norm of the solution and a few
+sampled solution entries).  Calls only oracle/ and the seeded input generators; nothing here
+touches the CUDA library.  Usage: python tests/golden/make_golden.py [cfg ...]   (default 1 2 3 4)
+
+The full-size GPU tests compare against these instead of re-running minutes of oracle CG.
+LAPACK rounding in the input generators may differ in the last bit between machines; the CG
+tolerances (solution 1e-9, iterations +-2) absorb that.
+"""
+import json
+import os
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+sys.path.insert(0, ROOT)
+
+import oracle  # noqa: E402
+from paper_1311_2719_b200 import synth  # noqa: E402
+
+OUT = os.path.join(os.path.dirname(os.path.abspath(__file__)), "oracle_cg_reference.json")
+NSAMPLE = 64
+
+
+def main():
+    cfgs = [int(a) for a in sys.argv[1:]] or [1, 2, 3, 4]
+    ref = json.load(open(OUT)) if os.path.exists(OUT) else {}
+    for n in cfgs:
+        c, u, b = synth.config_inputs(n)
+        f = 0 if c["fermion"] == "staggered" else 1
+        t0 = time.time()
+        r = oracle.cg(c["dims"], f, u, c["param"], c["tol"], 100000, b)
+        dt = time.time() - t0
+        x = r["x"].ravel()
+        idx = np.random.default_rng(1311 + n).choice(x.size, NSAMPLE, replace=False)
+        idx.sort()
+        ref["cfg%d" % n] = {
+            "dims": list(c["dims"]), "fermion": c["fermion"], "links": c["links"], "param": c["param"],
+            "tol": c["tol"], "seed": c["seed"], "iters": r["iters"], "status": r["status"],
+            "true_residual": r["true_residual"], "x_norm": float(np.linalg.norm(x)),
+            "sample_index": [int(i) for i in idx], "sample_re": [float(v) for v in x[idx].real],
+            "sample_im": [float(v) for v in x[idx].imag], "oracle_seconds": round(dt, 1),
+            "oracle_threads": oracle.num_threads(),
+        }
+        print("cfg%d: iters %d, true residual %.3e, %.1f s" % (n, r["iters"], r["true_residual"], dt), flush=True)
+        json.dump(ref, open(OUT, "w"), indent=1, sort_keys=True)
+
+
+if __name__ == "__main__":
+    main()
