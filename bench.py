@@ -186,38 +186,19 @@ def main():
 
     # ------------------------------------------------------------------ our arm
     import torch
-    import torch.distributed as dist
     from paper_1311_2719_b200 import lqcd
+    from paper_1311_2719_b200.ranks import Ranks
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the CUDA path is the only path")
     torch.cuda.set_device(local_rank)
     device = torch.device("cuda", local_rank)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=device)
-
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    def max_over_ranks(x: float) -> float:
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=device)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
-
-    def sum_over_ranks(x: float) -> float:
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=device)
-        dist.all_reduce(t, op=dist.ReduceOp.SUM)
-        return float(t.item())
+    ranks = Ranks(backend="nccl", device=device)
+    barrier, max_over_ranks, sum_over_ranks = ranks.barrier, ranks.max, ranks.sum
 
     f = lqcd.STAGGERED if cfg["fermion"] == "staggered" else lqcd.WILSON
     u = synth.gauge_field(cfg["dims"], cfg["links"], cfg["seed"])
-    b = synth.source(cfg["dims"], cfg["fermion"], cfg["seed"] + 1000 * rank)   # one right-hand side per rank
+    b = synth.source(cfg["dims"], cfg["fermion"], ranks.rhs_seed(cfg["seed"]))   # one right-hand side per rank
     u_host = torch.from_numpy(u).pin_memory()
     b_host = torch.from_numpy(b).pin_memory()
     lat = lqcd.Lattice(cfg["dims"], f, device=device)
@@ -321,8 +302,7 @@ def main():
         line["roofline"]["traffic"] = ncu_traffic("%s_dslash_plain" % cfg["name"])
         print(json.dumps(line))
     lat.close()
-    if world > 1:
-        dist.destroy_process_group()
+    ranks.close()
     return 0
 
 
