@@ -73,7 +73,17 @@ enum {
                           a device-side flag turns iterations after convergence into no-ops */
     LQCD_CG_GRAPH = 2  /* ASYNC with each batch of iterations replayed from one CUDA graph */
 };
-enum { LQCD_OPT_CG_MODE = 0, LQCD_OPT_CG_CHECK_EVERY = 1 };
+enum {
+    LQCD_OPT_CG_MODE = 0,
+    LQCD_OPT_CG_CHECK_EVERY = 1, /* iterations enqueued per convergence read-back, 1..1024 */
+    /* 18 (default): all nine complex entries of a link are stored and read (144 B per link).
+     * 12: only the first two rows are stored; the third is rebuilt in registers as the
+     * conjugated cross product (PAPER.md:132 names this "two-column link compression" as the
+     * optimisation its code does not use): 96 B per link, 864 instead of
+     * 1248 B per staggered Dslash site.  Exact for SU(3) links up to rounding (1e-16).
+     * Changing it invalidates the loaded gauge field: call lqcd_load_gauge again. */
+    LQCD_OPT_RECONSTRUCT = 2
+};
 
 /* Create a context for an L0 x L1 x L2 x L3 lattice (every extent even and >= 2; L = 2 is
  * legal: forward and backward neighbour coincide).  Host-only; touches no device. */

@@ -58,26 +58,29 @@ __global__ void __launch_bounds__(BLOCK) cg_pupdate_kernel(const cplx* __restric
     grid_sum<BLOCK>(local, rs, [sc](double pp) { sc->pp = pp; });
 }
 
-// S0: canonical u[g][mu][3][3] (array of structures, 576 B per site) -> [parity][mu][9][Vh]
-// (structure of arrays).  A block stages TILE sites through shared memory so both the global
-// read and the global write are contiguous.
-template <int BLOCK, int TILE>
-__global__ void __launch_bounds__(BLOCK) gauge_reorder_kernel(const cplx* __restrict__ u, cplx* __restrict__ soa,
+// S0: canonical u[g][mu][3][3] (array of structures, 576 B per site, fp64) ->
+// [parity][mu][RECON/2][Vh] in the storage type C (structure of arrays; two rows only for
+// RECON = 12).  A block stages TILE sites through shared memory so both the global read and the
+// global write are contiguous.
+template <int BLOCK, int TILE, int RECON, class C>
+__global__ void __launch_bounds__(BLOCK) gauge_reorder_kernel(const cplx* __restrict__ u, C* __restrict__ soa,
                                                               size_t Vh)
 {
+    constexpr int NC = RECON / 2;
     __shared__ cplx tile[TILE * 36 + 1];
     const size_t V = 2 * Vh;
     const size_t g0 = (size_t)blockIdx.x * TILE;
     const size_t nsite = g0 + TILE <= V ? TILE : V - g0;
     for (size_t i = threadIdx.x; i < nsite * 36; i += BLOCK) tile[i] = u[g0 * 36 + i];
     __syncthreads();
-    for (size_t i = threadIdx.x; i < nsite * 36; i += BLOCK) {
-        const size_t j = i / nsite;  // mu*9 + k
+    for (size_t i = threadIdx.x; i < nsite * 4 * NC; i += BLOCK) {
+        const size_t j = i / nsite;  // mu*NC + k
         const size_t s = i - j * nsite;
+        const size_t mu = j / NC, k = j - mu * NC;
         const size_t g = g0 + s;
         const size_t parity = g >= Vh ? 1 : 0;
         const size_t e = g - parity * Vh;
-        soa[(parity * 36 + j) * Vh + e] = tile[s * 36 + j];
+        soa[(parity * 4 * NC + j) * Vh + e] = to_cplx(tile[s * 36 + mu * 9 + k], (C*)0);
     }
 }
 

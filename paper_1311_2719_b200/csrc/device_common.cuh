@@ -1,12 +1,19 @@
-// device_common.cuh -- lattice geometry, complex arithmetic and cache-hinted loads shared by
-// the Dslash kernels.  Index convention: include/lqcd.h.
+// device_common.cuh -- lattice geometry, complex arithmetic, link loading (with the optional
+// two-row reconstruction) and cache-hinted loads shared by the Dslash kernels.
+// Index convention: include/lqcd.h.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
 
 namespace lqcd {
 
-typedef double2 cplx;  // (re, im): one 128-bit load/store per complex number
+// One complex number = one vector load/store: 128 bits in fp64, 64 bits in fp32 (the fp32
+// types serve the inner iterations of the mixed-precision solver only).
+template <class T> struct CplxOf;
+template <> struct CplxOf<double> { typedef double2 type; };
+template <> struct CplxOf<float> { typedef float2 type; };
+typedef double2 cplx;   // fp64 complex, the precision of the path (reading A5)
+typedef float2 cplxf;
 
 // Half-lattice geometry.  A site of parity p is addressed by e = xh + Lh*(x1 + L1*(x2 + L2*x3)),
 // xh = x0 >> 1, x0 = 2*xh + ((x1+x2+x3+p) & 1).
@@ -66,27 +73,51 @@ __device__ __forceinline__ double bc_bwd(const Geom& g, const Site& s)
     return (MU == 3 && s.x3 == 0) ? -1.0 : 1.0;
 }
 
+// Staggered phase eta_mu(x) / 2 (reading A3) from the decoded site.
+template <int MU>
+__device__ __forceinline__ double half_eta(const Site& s)
+{
+    if (MU == 0) return 0.5;
+    if (MU == 1) return s.r ? -0.5 : 0.5;
+    if (MU == 2) return ((s.r + s.x1) & 1) ? -0.5 : 0.5;
+    return ((s.r + s.x1 + s.x2) & 1) ? -0.5 : 0.5;
+}
+
 // ------------------------------------------------------------------ loads / stores
 // Links are read exactly once per Dslash and the field (0.6-6 GB) does not fit the 126 MB L2:
 // stream them (evict-first, no L1 allocation) so they do not push the vectors out.
-__device__ __forceinline__ cplx ld_stream(const cplx* p)
+__device__ __forceinline__ double2 ld_stream(const double2* p)
 {
-    cplx v;
+    double2 v;
     asm volatile("ld.global.cs.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
     return v;
 }
+__device__ __forceinline__ float2 ld_stream(const float2* p)
+{
+    float2 v;
+    asm volatile("ld.global.cs.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+    return v;
+}
 // Vectors are re-read by up to 8 neighbouring sites: read-only path, keep in L1/L2.
-__device__ __forceinline__ cplx ld_keep(const cplx* p) { return __ldg(p); }
-__device__ __forceinline__ void st_vec(cplx* p, cplx v) { *p = v; }
+__device__ __forceinline__ double2 ld_keep(const double2* p) { return __ldg(p); }
+__device__ __forceinline__ float2 ld_keep(const float2* p) { return __ldg(p); }
+template <class C>
+__device__ __forceinline__ void st_vec(C* p, C v) { *p = v; }
 
 // ------------------------------------------------------------------ complex helpers
-__device__ __forceinline__ cplx cmake(double re, double im) { return make_double2(re, im); }
-__device__ __forceinline__ cplx cadd(cplx a, cplx b) { return cmake(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ cplx csub(cplx a, cplx b) { return cmake(a.x - b.x, a.y - b.y); }
-__device__ __forceinline__ cplx cscale(double s, cplx a) { return cmake(s * a.x, s * a.y); }
-__device__ __forceinline__ double cnorm2(cplx a) { return fma(a.x, a.x, a.y * a.y); }
+__device__ __forceinline__ double2 cmake(double re, double im) { return make_double2(re, im); }
+__device__ __forceinline__ float2 cmake(float re, float im) { return make_float2(re, im); }
+template <class C> __device__ __forceinline__ C czero() { C z; z.x = 0; z.y = 0; return z; }
+template <class C> __device__ __forceinline__ C cadd(C a, C b) { return cmake(a.x + b.x, a.y + b.y); }
+template <class C> __device__ __forceinline__ C csub(C a, C b) { return cmake(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ double2 cscale(double s, double2 a) { return cmake(s * a.x, s * a.y); }
+__device__ __forceinline__ float2 cscale(double s, float2 a) { return cmake((float)s * a.x, (float)s * a.y); }
+// |a|^2, always returned (and summed by the caller) in fp64
+__device__ __forceinline__ double cnorm2(double2 a) { return fma(a.x, a.x, a.y * a.y); }
+__device__ __forceinline__ double cnorm2(float2 a) { return (double)a.x * (double)a.x + (double)a.y * (double)a.y; }
 // acc += a * b
-__device__ __forceinline__ void cfma(cplx& acc, cplx a, cplx b)
+template <class C>
+__device__ __forceinline__ void cfma(C& acc, C a, C b)
 {
     acc.x = fma(a.x, b.x, acc.x);
     acc.x = fma(-a.y, b.y, acc.x);
@@ -94,21 +125,63 @@ __device__ __forceinline__ void cfma(cplx& acc, cplx a, cplx b)
     acc.y = fma(a.y, b.x, acc.y);
 }
 // acc += conj(a) * b
-__device__ __forceinline__ void cfma_conj(cplx& acc, cplx a, cplx b)
+template <class C>
+__device__ __forceinline__ void cfma_conj(C& acc, C a, C b)
 {
     acc.x = fma(a.x, b.x, acc.x);
     acc.x = fma(a.y, b.y, acc.x);
     acc.y = fma(a.x, b.y, acc.y);
     acc.y = fma(-a.y, b.x, acc.y);
 }
+// conj(a*b - c*d)
+template <class C>
+__device__ __forceinline__ C conj_cross(C a, C b, C c, C d)
+{
+    C r;
+    r.x = fma(a.x, b.x, -(a.y * b.y));
+    r.x = fma(-c.x, d.x, r.x);
+    r.x = fma(c.y, d.y, r.x);
+    r.y = fma(c.x, d.y, c.y * d.x);
+    r.y = fma(-a.x, b.y, r.y);
+    r.y = fma(-a.y, b.x, r.y);
+    return r;
+}
 // multiplication by i^K
-template <int K>
-__device__ __forceinline__ cplx mul_i_pow(cplx a)
+template <int K, class C>
+__device__ __forceinline__ C mul_i_pow(C a)
 {
     if (K == 0) return a;
     if (K == 1) return cmake(-a.y, a.x);
     if (K == 2) return cmake(-a.x, -a.y);
     return cmake(a.y, -a.x);
+}
+// fp64 <-> working precision
+__device__ __forceinline__ double2 to_d(double2 a) { return a; }
+__device__ __forceinline__ double2 to_d(float2 a) { return make_double2((double)a.x, (double)a.y); }
+__device__ __forceinline__ double2 to_cplx(double2 a, double2*) { return a; }
+__device__ __forceinline__ float2 to_cplx(double2 a, float2*) { return make_float2((float)a.x, (float)a.y); }
+
+// ------------------------------------------------------------------ links
+// Internal gauge layout: [parity][mu][NC][Vh] with NC = RECON/2 stored complex numbers per link.
+// RECON = 18: all nine entries.  RECON = 12: the first two rows; the third row of an SU(3) matrix
+// is the conjugated cross product of the first two ("two-column link compression",
+// SURVEY.md 8(f) row 1): 96 instead of 144 bytes per link from HBM for 42 extra flops.
+template <int RECON, class C>
+__device__ __forceinline__ void load_link(const C* __restrict__ p, size_t Vh, C U[9])
+{
+    constexpr int NC = RECON / 2;
+#pragma unroll
+    for (int k = 0; k < NC; ++k) U[k] = ld_stream(p + k * Vh);
+}
+// Kept apart from load_link so that a hop can issue all its loads before the first dependent flop.
+template <int RECON, class C>
+__device__ __forceinline__ void reconstruct_link(C U[9])
+{
+    if (RECON == 12) {
+        U[6] = conj_cross(U[1], U[5], U[2], U[4]);
+        U[7] = conj_cross(U[2], U[3], U[0], U[5]);
+        U[8] = conj_cross(U[0], U[4], U[1], U[3]);
+    }
 }
 
 }  // namespace lqcd

@@ -24,6 +24,8 @@ constexpr int kVecBlock = 256;
 constexpr int kReorderTile = 64;
 constexpr size_t kAlign = 256;
 
+typedef StagArgs<cplx> StagArgsD;
+
 size_t align_up(size_t n) { return (n + kAlign - 1) / kAlign * kAlign; }
 
 }  // namespace
@@ -45,6 +47,7 @@ struct lqcd_ctx {
     // options
     int cg_mode;
     int check_every;
+    int recon;  // 18 or 12 stored reals per link
     // host side
     CgScalars* h_sc;  // pinned, 2 slots
     cudaEvent_t ev[2];
@@ -118,9 +121,9 @@ unsigned int vec_grid(const lqcd_ctx* ctx)
 }
 
 // ---------------------------------------------------------------- staggered launches
-StagArgs stag_args(const lqcd_ctx* ctx, int parity, const cplx* in, cplx* out)
+StagArgsD stag_args(const lqcd_ctx* ctx, int parity, const cplx* in, cplx* out)
 {
-    StagArgs a;
+    StagArgsD a;
     memset(&a, 0, sizeof a);
     a.g = ctx->g;
     a.parity = parity;
@@ -134,9 +137,13 @@ StagArgs stag_args(const lqcd_ctx* ctx, int parity, const cplx* in, cplx* out)
 }
 
 template <int EPI>
-int launch_stag(lqcd_ctx* ctx, const StagArgs& a)
+int launch_stag(lqcd_ctx* ctx, const StagArgsD& a)
 {
-    stag_dslash_kernel<EPI, kStagBlock><<<blocks_for(ctx->g.Vh, kStagBlock), kStagBlock, 0, ctx->stream>>>(a);
+    const unsigned int grid = blocks_for(ctx->g.Vh, kStagBlock);
+    if (ctx->recon == 12)
+        stag_dslash_kernel<EPI, kStagBlock, 12, cplx><<<grid, kStagBlock, 0, ctx->stream>>>(a);
+    else
+        stag_dslash_kernel<EPI, kStagBlock, 18, cplx><<<grid, kStagBlock, 0, ctx->stream>>>(a);
     LQCD_LAUNCH_CHECK();
     return LQCD_OK;
 }
@@ -162,7 +169,11 @@ template <int EPI, bool DAGGER>
 int launch_wilson(lqcd_ctx* ctx, const WilsonArgs& a)
 {
     const size_t n = EPI == WE_PLAIN ? (size_t)ctx->g.Vh : (size_t)ctx->g.V;
-    wilson_dslash_kernel<EPI, DAGGER, kWilsonBlock><<<blocks_for(n, kWilsonBlock), kWilsonBlock, 0, ctx->stream>>>(a);
+    const unsigned int grid = blocks_for(n, kWilsonBlock);
+    if (ctx->recon == 12)
+        wilson_dslash_kernel<EPI, DAGGER, kWilsonBlock, 12><<<grid, kWilsonBlock, 0, ctx->stream>>>(a);
+    else
+        wilson_dslash_kernel<EPI, DAGGER, kWilsonBlock, 18><<<grid, kWilsonBlock, 0, ctx->stream>>>(a);
     LQCD_LAUNCH_CHECK();
     return LQCD_OK;
 }
@@ -172,7 +183,7 @@ int launch_wilson(lqcd_ctx* ctx, const WilsonArgs& a)
 int op_first(lqcd_ctx* ctx, double param, const cplx* v, bool with_norm)
 {
     if (ctx->fermion == LQCD_STAGGERED) {
-        StagArgs a = stag_args(ctx, LQCD_ODD, v, ctx->t());
+        StagArgsD a = stag_args(ctx, LQCD_ODD, v, ctx->t());
         a.m2 = param * param;
         return with_norm ? launch_stag<SE_NORM>(ctx, a) : launch_stag<SE_PLAIN>(ctx, a);
     }
@@ -185,7 +196,7 @@ int cg_iteration_kernels(lqcd_ctx* ctx, double param, cplx* x)
     int rc = op_first(ctx, param, ctx->p(), true);  // S1 + S2
     if (rc) return rc;
     if (ctx->fermion == LQCD_STAGGERED) {           // S3
-        StagArgs a = stag_args(ctx, LQCD_EVEN, ctx->t(), nullptr);
+        StagArgsD a = stag_args(ctx, LQCD_EVEN, ctx->t(), nullptr);
         a.m2 = param * param;
         a.p = ctx->p();
         a.x = x;
@@ -279,6 +290,7 @@ int lqcd_create(lqcd_ctx** out, int L0, int L1, int L2, int L3, int fermion_type
     c->max_blocks = (size_t)V / 64 + 4096;
     c->cg_mode = LQCD_CG_ASYNC;
     c->check_every = 4;
+    c->recon = 18;
 
     size_t off = 0;
     const size_t vec_bytes = align_up(c->nvec * sizeof(cplx));
@@ -349,6 +361,12 @@ int lqcd_set_option(lqcd_ctx* ctx, int option, int value)
         ctx->check_every = value;
         return LQCD_OK;
     }
+    if (option == LQCD_OPT_RECONSTRUCT) {
+        if (value != 18 && value != 12) return fail(ctx, LQCD_EARG, "reconstruct must be 18 or 12");
+        if (value != ctx->recon) ctx->gauge_loaded = false;  // the internal copy has the other layout
+        ctx->recon = value;
+        return LQCD_OK;
+    }
     return fail(ctx, LQCD_EARG, "unknown option %d", option);
 }
 
@@ -358,8 +376,13 @@ int lqcd_load_gauge(lqcd_ctx* ctx, const double* u_dev)
     if (rc) return rc;
     if (!u_dev) return fail(ctx, LQCD_EARG, "u_dev is null");
     const size_t V = (size_t)ctx->g.V;
-    gauge_reorder_kernel<256, kReorderTile><<<blocks_for(V, kReorderTile), 256, 0, ctx->stream>>>(
-        (const cplx*)u_dev, ctx->gauge(), (size_t)ctx->g.Vh);
+    const unsigned int grid = blocks_for(V, kReorderTile);
+    if (ctx->recon == 12)
+        gauge_reorder_kernel<256, kReorderTile, 12, cplx><<<grid, 256, 0, ctx->stream>>>((const cplx*)u_dev, ctx->gauge(),
+                                                                                         (size_t)ctx->g.Vh);
+    else
+        gauge_reorder_kernel<256, kReorderTile, 18, cplx><<<grid, 256, 0, ctx->stream>>>((const cplx*)u_dev, ctx->gauge(),
+                                                                                         (size_t)ctx->g.Vh);
     LQCD_LAUNCH_CHECK();
     ctx->gauge_loaded = true;
     return LQCD_OK;
@@ -402,7 +425,7 @@ int lqcd_apply_MdagM(lqcd_ctx* ctx, double mass_or_kappa, const double* in_dev, 
     rc = op_first(ctx, mass_or_kappa, (const cplx*)in_dev, false);
     if (rc) return rc;
     if (ctx->fermion == LQCD_STAGGERED) {
-        StagArgs a = stag_args(ctx, LQCD_EVEN, ctx->t(), (cplx*)out_dev);
+        StagArgsD a = stag_args(ctx, LQCD_EVEN, ctx->t(), (cplx*)out_dev);
         a.m2 = mass_or_kappa * mass_or_kappa;
         a.p = (const cplx*)in_dev;
         return launch_stag<SE_MDAGM>(ctx, a);
@@ -500,7 +523,7 @@ int lqcd_cg_solve(lqcd_ctx* ctx, double mass_or_kappa, double tol, int maxiter, 
     rc = op_first(ctx, mass_or_kappa, x, false);
     if (rc) return rc;
     if (ctx->fermion == LQCD_STAGGERED) {
-        StagArgs a = stag_args(ctx, LQCD_EVEN, ctx->t(), nullptr);
+        StagArgsD a = stag_args(ctx, LQCD_EVEN, ctx->t(), nullptr);
         a.m2 = mass_or_kappa * mass_or_kappa;
         a.p = x;
         a.b = b;

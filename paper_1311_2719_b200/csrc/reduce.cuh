@@ -37,6 +37,20 @@ struct ReduceScratch {
 
 static constexpr int kHistCap = 65536;
 
+// Scalar bookkeeping after x += alpha p, r -= alpha Ap (run by one thread of the last block):
+// iteration count, history, beta = betan/betad and betad = betan, exit flag
+// (relative rule, reading A6).
+__device__ __forceinline__ void cg_after_update(CgScalars* sc, double* hist, double rr_new)
+{
+    const int it = sc->iter + 1;
+    sc->iter = it;
+    sc->rr_new = rr_new;
+    if (it < kHistCap) hist[it] = rr_new;
+    sc->beta = rr_new / sc->rr;
+    sc->rr = rr_new;
+    if (rr_new <= sc->thresh || it >= sc->maxiter) sc->done = 1;
+}
+
 template <int BLOCK>
 __device__ __forceinline__ double block_sum(double v)
 {

@@ -26,46 +26,43 @@ enum StagEpilogue {
     SE_RESIDUAL = 4   // |b - (m^2 p - D in)|^2                                 (S7), nothing stored
 };
 
+template <class C>
 struct StagArgs {
     Geom g;
-    int parity;         // parity of the output sites
-    const cplx* gauge;  // [2][4][9][Vh]
-    const cplx* in;     // [3][Vh] on parity 1-parity
-    cplx* out;          // [3][Vh]
-    const cplx* p;      // epilogue operand on the output parity (p, or x for SE_RESIDUAL)
-    cplx* x;
-    cplx* r;
-    const cplx* b;
+    int parity;      // parity of the output sites
+    const C* gauge;  // [2][4][RECON/2][Vh]
+    const C* in;     // [3][Vh] on parity 1-parity
+    C* out;          // [3][Vh]
+    const C* p;      // epilogue operand on the output parity (p, or x for SE_RESIDUAL)
+    C* x;
+    C* r;
+    const C* b;
     double m2;
     CgScalars* sc;
     ReduceScratch rs;
     double* hist;
 };
 
-template <int MU>
-__device__ __forceinline__ void stag_hop(const StagArgs& a, const Site& s, cplx acc[3])
+template <int MU, int RECON, class C>
+__device__ __forceinline__ void stag_hop(const StagArgs<C>& a, const Site& s, C acc[3])
 {
+    constexpr int NC = RECON / 2;
     const size_t Vh = (size_t)a.g.Vh;
-    double eta;
-    if (MU == 0) eta = 0.5;
-    else if (MU == 1) eta = s.r ? -0.5 : 0.5;
-    else if (MU == 2) eta = ((s.r + s.x1) & 1) ? -0.5 : 0.5;
-    else eta = ((s.r + s.x1 + s.x2) & 1) ? -0.5 : 0.5;
-
+    const double eta = half_eta<MU>(s);
     const int ef = nbr_fwd<MU>(a.g, s);
     const int eb = nbr_bwd<MU>(a.g, s);
-    const cplx* Uf = a.gauge + (size_t)((a.parity * 4 + MU) * 9) * Vh + s.e;
-    const cplx* Ub = a.gauge + (size_t)(((1 - a.parity) * 4 + MU) * 9) * Vh + eb;
+    const C* Uf = a.gauge + (size_t)((a.parity * 4 + MU) * NC) * Vh + s.e;
+    const C* Ub = a.gauge + (size_t)(((1 - a.parity) * 4 + MU) * NC) * Vh + eb;
 
-    cplx U[9], W[9], vf[3], vb[3];
-#pragma unroll
-    for (int k = 0; k < 9; ++k) U[k] = ld_stream(Uf + k * Vh);
+    C U[9], W[9], vf[3], vb[3];
+    load_link<RECON>(Uf, Vh, U);
 #pragma unroll
     for (int c = 0; c < 3; ++c) vf[c] = ld_keep(a.in + c * Vh + ef);
-#pragma unroll
-    for (int k = 0; k < 9; ++k) W[k] = ld_stream(Ub + k * Vh);
+    load_link<RECON>(Ub, Vh, W);
 #pragma unroll
     for (int c = 0; c < 3; ++c) vb[c] = ld_keep(a.in + c * Vh + eb);
+    reconstruct_link<RECON>(U);
+    reconstruct_link<RECON>(W);
 
     const double sf = eta * bc_fwd<MU>(a.g, s);
     const double sb = -eta * bc_bwd<MU>(a.g, s);
@@ -84,8 +81,19 @@ __device__ __forceinline__ void stag_hop(const StagArgs& a, const Site& s, cplx 
     }
 }
 
-template <int EPI, int BLOCK>
-__global__ void __launch_bounds__(BLOCK) stag_dslash_kernel(const StagArgs a)
+// Epilogue arithmetic is done in fp64 whatever the storage type C (free for fp64, a handful of
+// converts per site for the fp32 inner iterations of the mixed-precision solver).
+// Minimum resident blocks per SM.  Two-row links: without a bound ptxas keeps both links of a hop
+// and their rebuilt rows live (128-138 registers, 3 blocks/SM: 6.2 TB/s); 4 blocks/SM caps it at
+// 128 and measured best on B200 (65.4 us at 32^4 = 6.9 TB/s; 5 -> 68 us, 6+ spills -> 100+ us).
+#ifndef LQCD_STAG_MINB18
+#define LQCD_STAG_MINB18 1
+#endif
+#ifndef LQCD_STAG_MINB12
+#define LQCD_STAG_MINB12 4
+#endif
+template <int EPI, int BLOCK, int RECON, class C>
+__global__ void __launch_bounds__(BLOCK, RECON == 12 ? LQCD_STAG_MINB12 : LQCD_STAG_MINB18) stag_dslash_kernel(const StagArgs<C> a)
 {
     if (EPI == SE_NORM || EPI == SE_CGUPDATE) {
         if (a.sc->done) return;  // converged earlier: this (pre-enqueued) iteration is a no-op
@@ -93,13 +101,13 @@ __global__ void __launch_bounds__(BLOCK) stag_dslash_kernel(const StagArgs a)
     const int e = blockIdx.x * BLOCK + threadIdx.x;
     const bool active = e < a.g.Vh;
     const size_t Vh = (size_t)a.g.Vh;
-    cplx acc[3] = { cmake(0, 0), cmake(0, 0), cmake(0, 0) };
+    C acc[3] = { czero<C>(), czero<C>(), czero<C>() };
     if (active) {
         const Site s = decode_site(a.g, a.parity, e);
-        stag_hop<0>(a, s, acc);
-        stag_hop<1>(a, s, acc);
-        stag_hop<2>(a, s, acc);
-        stag_hop<3>(a, s, acc);
+        stag_hop<0, RECON>(a, s, acc);
+        stag_hop<1, RECON>(a, s, acc);
+        stag_hop<2, RECON>(a, s, acc);
+        stag_hop<3, RECON>(a, s, acc);
     }
     if (EPI == SE_PLAIN) {
         if (active) {
@@ -110,8 +118,8 @@ __global__ void __launch_bounds__(BLOCK) stag_dslash_kernel(const StagArgs a)
         if (active) {
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
-                const cplx pv = a.p[c * Vh + e];
-                st_vec(a.out + c * Vh + e, cmake(fma(a.m2, pv.x, -acc[c].x), fma(a.m2, pv.y, -acc[c].y)));
+                const double2 pv = to_d(a.p[c * Vh + e]), q = to_d(acc[c]);
+                st_vec(a.out + c * Vh + e, to_cplx(cmake(fma(a.m2, pv.x, -q.x), fma(a.m2, pv.y, -q.y)), (C*)0));
             }
         }
     } else if (EPI == SE_NORM) {
@@ -136,38 +144,31 @@ __global__ void __launch_bounds__(BLOCK) stag_dslash_kernel(const StagArgs a)
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
                 const size_t i = c * Vh + e;
-                const cplx pv = a.p[i];
-                cplx xv = a.x[i], rv = a.r[i];
-                const cplx ap = cmake(fma(a.m2, pv.x, -acc[c].x), fma(a.m2, pv.y, -acc[c].y));
+                const double2 pv = to_d(a.p[i]), q = to_d(acc[c]);
+                double2 xv = to_d(a.x[i]), rv = to_d(a.r[i]);
+                const double2 ap = cmake(fma(a.m2, pv.x, -q.x), fma(a.m2, pv.y, -q.y));
                 xv.x = fma(alpha, pv.x, xv.x);   // x = x + alpha p
                 xv.y = fma(alpha, pv.y, xv.y);
                 rv.x = fma(-alpha, ap.x, rv.x);  // r = r - alpha atap
                 rv.y = fma(-alpha, ap.y, rv.y);
-                a.x[i] = xv;
-                a.r[i] = rv;
-                local += cnorm2(rv);             // betan = <r,r>
+                const C rs_ = to_cplx(rv, (C*)0);
+                a.x[i] = to_cplx(xv, (C*)0);
+                a.r[i] = rs_;
+                local += cnorm2(rs_);            // betan = <r,r>
             }
         }
         CgScalars* sc = a.sc;
         double* hist = a.hist;
-        grid_sum<BLOCK>(local, a.rs, [sc, hist](double rr_new) {
-            const int it = sc->iter + 1;
-            sc->iter = it;
-            sc->rr_new = rr_new;
-            if (it < kHistCap) hist[it] = rr_new;
-            sc->beta = rr_new / sc->rr;  // beta = betan/betad; betad = betan
-            sc->rr = rr_new;
-            if (rr_new <= sc->thresh || it >= sc->maxiter) sc->done = 1;
-        });
+        grid_sum<BLOCK>(local, a.rs, [sc, hist](double rr_new) { cg_after_update(sc, hist, rr_new); });
     } else {  // SE_RESIDUAL
         double local = 0.0;
         if (active) {
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
                 const size_t i = c * Vh + e;
-                const cplx xv = a.p[i], bv = a.b[i];
-                const double re = bv.x - fma(a.m2, xv.x, -acc[c].x);
-                const double im = bv.y - fma(a.m2, xv.y, -acc[c].y);
+                const double2 xv = to_d(a.p[i]), bv = to_d(a.b[i]), q = to_d(acc[c]);
+                const double re = bv.x - fma(a.m2, xv.x, -q.x);
+                const double im = bv.y - fma(a.m2, xv.y, -q.y);
                 local += fma(re, re, im * im);
             }
         }

@@ -28,7 +28,7 @@ enum WilsonEpilogue {
 struct WilsonArgs {
     Geom g;
     int parity;         // WE_PLAIN: output parity.  Other epilogues cover both parities.
-    const cplx* gauge;  // [2][4][9][Vh]
+    const cplx* gauge;  // [2][4][RECON/2][Vh]
     const cplx* in;     // [4][3][V]
     cplx* out;          // [4][3][V]
     const cplx* p;
@@ -50,18 +50,18 @@ template <> struct GammaDR<3> { static constexpr int PI0 = 2, K0 = 0, PI1 = 3, K
 
 // One hop.  PLUS = false: projector (1 - gamma_mu); PLUS = true: (1 + gamma_mu).
 // ADJ = false: multiply by U (forward link at x); ADJ = true: by U^+ (link at x - mu^).
-template <int MU, bool PLUS, bool ADJ>
+template <int MU, bool PLUS, bool ADJ, int RECON>
 __device__ __forceinline__ void wilson_hop(const cplx* __restrict__ link, size_t Vh, const cplx* __restrict__ src,
                                            size_t V, double sign, cplx acc[4][3])
 {
     typedef GammaDR<MU> G;
     cplx U[9], psi[4][3];
-#pragma unroll
-    for (int k = 0; k < 9; ++k) U[k] = ld_stream(link + k * Vh);
+    load_link<RECON>(link, Vh, U);
 #pragma unroll
     for (int s = 0; s < 4; ++s)
 #pragma unroll
         for (int c = 0; c < 3; ++c) psi[s][c] = ld_keep(src + (size_t)(s * 3 + c) * V);
+    reconstruct_link<RECON>(U);
 
     // h_s = psi_s -+ i^K psi_pi(s)
     constexpr int KH0 = PLUS ? G::K0 : (G::K0 + 2) & 3;
@@ -77,7 +77,7 @@ __device__ __forceinline__ void wilson_hop(const cplx* __restrict__ link, size_t
     }
 #pragma unroll
     for (int r = 0; r < 3; ++r) {
-        cplx u0 = cmake(0, 0), u1 = cmake(0, 0);
+        cplx u0 = czero<cplx>(), u1 = czero<cplx>();
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
             if (ADJ) {
@@ -95,21 +95,21 @@ __device__ __forceinline__ void wilson_hop(const cplx* __restrict__ link, size_t
     }
 }
 
-template <int MU, bool DAGGER>
+template <int MU, bool DAGGER, int RECON>
 __device__ __forceinline__ void wilson_dir(const WilsonArgs& a, const Site& s, int parity, cplx acc[4][3])
 {
     const size_t Vh = (size_t)a.g.Vh, V = (size_t)a.g.V;
     const int ef = nbr_fwd<MU>(a.g, s);
     const int eb = nbr_bwd<MU>(a.g, s);
     const size_t other = (size_t)(1 - parity) * Vh;
-    const cplx* Uf = a.gauge + (size_t)((parity * 4 + MU) * 9) * Vh + s.e;
-    const cplx* Ub = a.gauge + (size_t)(((1 - parity) * 4 + MU) * 9) * Vh + eb;
+    const cplx* Uf = a.gauge + (size_t)((parity * 4 + MU) * (RECON / 2)) * Vh + s.e;
+    const cplx* Ub = a.gauge + (size_t)(((1 - parity) * 4 + MU) * (RECON / 2)) * Vh + eb;
     // D: forward (1-gamma), backward (1+gamma);  D^+: forward (1+gamma), backward (1-gamma)
-    wilson_hop<MU, DAGGER, false>(Uf, Vh, a.in + other + ef, V, bc_fwd<MU>(a.g, s), acc);
-    wilson_hop<MU, !DAGGER, true>(Ub, Vh, a.in + other + eb, V, bc_bwd<MU>(a.g, s), acc);
+    wilson_hop<MU, DAGGER, false, RECON>(Uf, Vh, a.in + other + ef, V, bc_fwd<MU>(a.g, s), acc);
+    wilson_hop<MU, !DAGGER, true, RECON>(Ub, Vh, a.in + other + eb, V, bc_bwd<MU>(a.g, s), acc);
 }
 
-template <int EPI, bool DAGGER, int BLOCK>
+template <int EPI, bool DAGGER, int BLOCK, int RECON>
 __global__ void __launch_bounds__(BLOCK) wilson_dslash_kernel(const WilsonArgs a)
 {
     if (EPI == WE_M_NORM || EPI == WE_CGUPDATE) {
@@ -134,13 +134,13 @@ __global__ void __launch_bounds__(BLOCK) wilson_dslash_kernel(const WilsonArgs a
 #pragma unroll
     for (int s = 0; s < 4; ++s)
 #pragma unroll
-        for (int c = 0; c < 3; ++c) acc[s][c] = cmake(0, 0);
+        for (int c = 0; c < 3; ++c) acc[s][c] = czero<cplx>();
     if (active) {
         const Site st = decode_site(a.g, parity, e);
-        wilson_dir<0, DAGGER>(a, st, parity, acc);
-        wilson_dir<1, DAGGER>(a, st, parity, acc);
-        wilson_dir<2, DAGGER>(a, st, parity, acc);
-        wilson_dir<3, DAGGER>(a, st, parity, acc);
+        wilson_dir<0, DAGGER, RECON>(a, st, parity, acc);
+        wilson_dir<1, DAGGER, RECON>(a, st, parity, acc);
+        wilson_dir<2, DAGGER, RECON>(a, st, parity, acc);
+        wilson_dir<3, DAGGER, RECON>(a, st, parity, acc);
     }
 
     if (EPI == WE_PLAIN) {
@@ -187,15 +187,7 @@ __global__ void __launch_bounds__(BLOCK) wilson_dslash_kernel(const WilsonArgs a
         });
     } else if (EPI == WE_CGUPDATE) {
         double* hist = a.hist;
-        grid_sum<BLOCK>(local, a.rs, [sc, hist](double rr_new) {
-            const int it = sc->iter + 1;
-            sc->iter = it;
-            sc->rr_new = rr_new;
-            if (it < kHistCap) hist[it] = rr_new;
-            sc->beta = rr_new / sc->rr;
-            sc->rr = rr_new;
-            if (rr_new <= sc->thresh || it >= sc->maxiter) sc->done = 1;
-        });
+        grid_sum<BLOCK>(local, a.rs, [sc, hist](double rr_new) { cg_after_update(sc, hist, rr_new); });
     } else if (EPI == WE_RESIDUAL) {
         grid_sum<BLOCK>(local, a.rs, [sc](double res2) { sc->res2 = res2; });
     }

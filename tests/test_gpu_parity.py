@@ -44,8 +44,9 @@ def fermion_name(f):
     return "staggered" if f == 0 else "wilson"
 
 
-def make_lattice(lq, dims, fermion, u):
+def make_lattice(lq, dims, fermion, u, recon=18):
     lat = lq.Lattice(dims, fermion)
+    lat.set_option(lq.OPT_RECONSTRUCT, recon)
     lat.load_gauge(dev(u))
     return lat
 
@@ -77,10 +78,11 @@ def test_tables_bit_exact_cfg5(lq):
 @pytest.mark.parametrize("dims", SMALL_SHAPES)
 @pytest.mark.parametrize("fermion", [0, 1])
 @pytest.mark.parametrize("kind", ["haar", "smooth"])
-def test_dslash_and_MdagM_small(lq, dims, fermion, kind):
+@pytest.mark.parametrize("recon", [18, 12])
+def test_dslash_and_MdagM_small(lq, dims, fermion, kind, recon):
     u = synth.gauge_field(dims, kind, 101)
     shape = oracle._vec_shape(dims, fermion)
-    with make_lattice(lq, dims, fermion, u) as lat:
+    with make_lattice(lq, dims, fermion, u, recon) as lat:
         for parity in (0, 1):
             vin = synth.vector(shape, 102 + parity)
             want = oracle.dslash(dims, fermion, u, parity, vin)
@@ -98,10 +100,11 @@ def test_dslash_and_MdagM_small(lq, dims, fermion, kind):
 
 
 @pytest.mark.parametrize("cfg", [1, 2, 3, 4])
-def test_dslash_configs_full_comparison(lq, cfg):
+@pytest.mark.parametrize("recon", [18, 12])
+def test_dslash_configs_full_comparison(lq, cfg, recon):
     c, u, b = synth.config_inputs(cfg)
     f = 0 if c["fermion"] == "staggered" else 1
-    with make_lattice(lq, c["dims"], f, u) as lat:
+    with make_lattice(lq, c["dims"], f, u, recon) as lat:
         for parity in (0, 1):
             vin = b if f == 1 else synth.vector(b.shape, 200 + parity)
             want = oracle.dslash(c["dims"], f, u, parity, vin)
@@ -146,12 +149,13 @@ def run_cg(lat, c, b, mode=None, maxiter=20000, tol=None):
 
 
 @pytest.mark.parametrize("cfg", [1, 2, 4])
-def test_cg_matches_oracle(lq, cfg):
+@pytest.mark.parametrize("recon", [18, 12])
+def test_cg_matches_oracle(lq, cfg, recon):
     c, u, b = synth.config_inputs(cfg)
     f = 0 if c["fermion"] == "staggered" else 1
     want = oracle.cg(c["dims"], f, u, c["param"], c["tol"], 20000, b, history=True)
     assert want["status"] == 0
-    with make_lattice(lq, c["dims"], f, u) as lat:
+    with make_lattice(lq, c["dims"], f, u, recon) as lat:
         x, it, res, status = run_cg(lat, c, b)
         hist = lat.cg_history().numpy()
     assert status == 0
@@ -256,13 +260,29 @@ def _check_against_golden(c, u, b, x, it, res, ref):
     assert res <= 2 * c["tol"]
 
 
+def test_reconstruct_option_invalidates_loaded_gauge(lq):
+    c, u, b = synth.config_inputs(1)
+    with make_lattice(lq, c["dims"], 0, u) as lat:
+        lat.set_option(lq.OPT_RECONSTRUCT, 18)        # unchanged: still loaded
+        lat.dslash(1, dev(b))
+        lat.set_option(lq.OPT_RECONSTRUCT, 12)
+        with pytest.raises(lq.LqcdError) as e:
+            lat.dslash(1, dev(b))
+        assert e.value.code == -3
+        with pytest.raises(lq.LqcdError):
+            lat.set_option(lq.OPT_RECONSTRUCT, 8)
+        lat.load_gauge(dev(u))
+        assert rel(host(lat.dslash(1, dev(b))), oracle.dslash(c["dims"], 0, u, 1, b)) <= DSLASH_TOL
+
+
 @pytest.mark.slow
-def test_cg_cfg3_bench_workload(lq):
+@pytest.mark.parametrize("recon", [18, 12])
+def test_cg_cfg3_bench_workload(lq, recon):
     """32^4, m = 0.01 in the launch configuration bench.py times.  The oracle's own solve takes
     minutes, so its iteration count and sampled solution entries are stored (make_golden.py);
     the solution is also checked here with one oracle application of A (holds at any size)."""
     c, u, b = synth.config_inputs(3)
-    with make_lattice(lq, c["dims"], 0, u) as lat:
+    with make_lattice(lq, c["dims"], 0, u, recon) as lat:
         x, it, res, status = run_cg(lat, c, b, maxiter=50000)
     assert status == 0 and res <= 2 * c["tol"]
     ax = oracle.apply_MdagM(c["dims"], 0, u, c["param"], x)
