@@ -40,17 +40,18 @@ NOMINAL_HBM_GBS = 8000.0
 FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
 
 
-def cg_bytes(cfg, iters: int) -> float:
-    """Algorithmic HBM bytes of one solve."""
+def cg_bytes(cfg, iters: int, recon: int = 18) -> float:
+    """Algorithmic HBM bytes of one solve; links cost 8 x recon x 8 B per site."""
     v = synth.volume(cfg["dims"])
+    links = 8 * recon * 8                                 # 1152 B (all nine entries) or 768 B (two rows)
     if cfg["fermion"] == "staggered":
         vh, vec = v // 2, 48
-        per_iter = 2 * 1152 + 11 * vec                    # 2832 B / site / iteration
-        fixed = 4 * vec + (1152 + 2 * vec) + (1152 + 4 * vec)  # init + D_oe x + fused residual
+        per_iter = 2 * links + 11 * vec                   # 2832 B / site / iteration at recon 18
+        fixed = 4 * vec + (links + 2 * vec) + (links + 4 * vec)  # init + D_oe x + fused residual
         return float(vh) * (per_iter * iters + fixed)
     vec = 192
-    per_iter = 2 * 1152 + 11 * vec                        # two full-lattice hops + 11 vector passes
-    fixed = 4 * vec + (1152 + 2 * vec) + (1152 + 3 * vec)
+    per_iter = 2 * links + 11 * vec                       # two full-lattice hops + 11 vector passes
+    fixed = 4 * vec + (links + 2 * vec) + (links + 3 * vec)
     return float(v) * (per_iter * iters + fixed)
 
 
@@ -152,6 +153,8 @@ def main():
     ap.add_argument("--cg-mode", default="graph", choices=["sync", "async", "graph"])
     ap.add_argument("--check-every", type=int, default=8)
     ap.add_argument("--dslash-reps", type=int, default=200)
+    ap.add_argument("--recon", type=int, default=18, choices=[18, 12],
+                    help="stored reals per link: 18 = all nine entries (the roofline workload), 12 = two rows")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -204,6 +207,7 @@ def main():
     lat = lqcd.Lattice(cfg["dims"], f, device=device)
     lat.set_option(lqcd.OPT_CG_MODE, {"sync": lqcd.CG_SYNC, "async": lqcd.CG_ASYNC, "graph": lqcd.CG_GRAPH}[args.cg_mode])
     lat.set_option(lqcd.OPT_CG_CHECK_EVERY, args.check_every)
+    lat.set_option(lqcd.OPT_RECONSTRUCT, args.recon)
     u_dev = u_host.to(device, non_blocking=True)
     b_dev = b_host.to(device, non_blocking=True)
     lat.load_gauge(u_dev)
@@ -230,7 +234,7 @@ def main():
     barrier()
     ms_solve = max_over_ranks(e0.elapsed_time(e1)) / args.steps
     launches = lat.kernel_launches() - launches0
-    total_bytes = sum_over_ranks(cg_bytes(cfg, iters))
+    total_bytes = sum_over_ranks(cg_bytes(cfg, iters, args.recon))
     value = total_bytes / (ms_solve * 1e-3) / 1e9
 
     # ---- timed region 2: the dominant kernel alone (plain Dslash), CUDA events on its stream.
@@ -238,12 +242,12 @@ def main():
     if f == lqcd.STAGGERED:
         va, vb = lat.new_vector(), lat.new_vector()
         va.copy_(b_dev)
-        dbytes, dflops = STAG_DSLASH_BYTES, STAG_DSLASH_FLOPS
+        dbytes, dflops = STAG_DSLASH_BYTES - 8 * 8 * (18 - args.recon), STAG_DSLASH_FLOPS
     else:
         va, vb = lat.new_vector(), lat.new_vector()
         va.copy_(b_dev)
         vb.zero_()
-        dbytes, dflops = WILSON_DSLASH_BYTES, WILSON_DSLASH_FLOPS
+        dbytes, dflops = WILSON_DSLASH_BYTES - 8 * 8 * (18 - args.recon), WILSON_DSLASH_FLOPS
     for i in range(6):
         lat.dslash(1 - (i & 1), va if not (i & 1) else vb, vb if not (i & 1) else va)
     d0, d1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -270,7 +274,7 @@ def main():
             _, it_e, res_e, st_e = lat.congrad_host(u_host, cfg["param"], cfg["tol"], maxiter, b_host, x_host)
         torch.cuda.synchronize()
         sec = max_over_ranks(time.perf_counter() - t0) / n_e2e
-        e2e = {"value": sum_over_ranks(cg_bytes(cfg, it_e)) / sec / 1e9, "unit": "GB/s", "ms_per_step": sec * 1e3,
+        e2e = {"value": sum_over_ranks(cg_bytes(cfg, it_e, args.recon)) / sec / 1e9, "unit": "GB/s", "ms_per_step": sec * 1e3,
                "h2d_bytes_per_step": int(u_host.numel() * 16 + b_host.numel() * 16),
                "d2h_bytes_per_step": int(x_host.numel() * 16 + 96), "iters": it_e, "true_residual": res_e,
                "api": "lqcd_congrad_host (pinned host u, b -> x)"}
@@ -286,7 +290,7 @@ def main():
             "metric": metric, "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_solve, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": workload, "cg_mode": args.cg_mode, "check_every": args.check_every,
+            "config": {"workload": workload, "reconstruct": args.recon, "cg_mode": args.cg_mode, "check_every": args.check_every,
                        "parallelism": "replicas x%d (independent right-hand sides)" % world,
                        "l2_policy": "inputs larger than L2 (%.0f MB of links per Dslash), no flush" % (v * 576 / 1e6)},
             "cg": {"time_to_solution_ms": ms_solve, "iters": iters, "true_residual": res,
@@ -299,7 +303,7 @@ def main():
                          "bytes_per_site": dbytes, "sites_per_launch": sites_out},
             "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "cpu_baseline": cpu,
         }
-        line["roofline"]["traffic"] = ncu_traffic("%s_dslash_plain" % cfg["name"])
+        line["roofline"]["traffic"] = ncu_traffic("%s_dslash_plain%s" % (cfg["name"], "" if args.recon == 18 else "_recon12"))
         print(json.dumps(line))
     lat.close()
     ranks.close()

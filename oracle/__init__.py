@@ -55,6 +55,8 @@ def lib():
         L.oracle_dot_re.argtypes = [P, P, ctypes.c_long]
         L.oracle_dot_re.restype = ctypes.c_double
         L.oracle_cg.argtypes = [P, ctypes.c_int, P, ctypes.c_double, ctypes.c_double, ctypes.c_int, P, P, P, P, P]
+        L.oracle_stag_M.argtypes = [P, P, ctypes.c_double, P, P, P, P]
+        L.oracle_stag_solve_full.argtypes = [P, P, ctypes.c_double, ctypes.c_double, ctypes.c_int, P, P, P, P, P, P]
         L.oracle_num_threads.restype = ctypes.c_int
         L.oracle_set_threads.argtypes = [ctypes.c_int]
         _lib = L
@@ -178,3 +180,32 @@ def cg(dims, fermion, u, param, tol, maxiter, b, history=False):
     if history:
         out["rr_history"] = hist[: it.value + 1]
     return out
+
+
+def stag_M(dims, u, mass, in_e, in_o):
+    """(M in)_e, (M in)_o with M = m + D on a full-lattice staggered vector given as its two halves."""
+    d = _dims(dims)
+    u = _c(u, np.complex128)
+    in_e = _c(in_e, np.complex128)
+    in_o = _c(in_o, np.complex128)
+    assert in_e.shape == _vec_shape(dims, STAGGERED) and in_o.shape == in_e.shape
+    out_e, out_o = np.empty_like(in_e), np.empty_like(in_o)
+    _check(lib().oracle_stag_M(_ptr(d), _ptr(u), float(mass), _ptr(in_e), _ptr(in_o), _ptr(out_e), _ptr(out_o)),
+           "oracle_stag_M")
+    return out_e, out_o
+
+
+def stag_solve_full(dims, u, mass, tol, maxiter, b_e, b_o):
+    """M x = b on the full lattice by even-odd reduction: dict(x_e, x_o, iters, true_residual, status)."""
+    d = _dims(dims)
+    u = _c(u, np.complex128)
+    b_e = _c(b_e, np.complex128)
+    b_o = _c(b_o, np.complex128)
+    assert b_e.shape == _vec_shape(dims, STAGGERED) and b_o.shape == b_e.shape
+    x_e, x_o = np.empty_like(b_e), np.empty_like(b_o)
+    it = ctypes.c_int(0)
+    res = ctypes.c_double(0.0)
+    rc = _check(lib().oracle_stag_solve_full(_ptr(d), _ptr(u), float(mass), float(tol), int(maxiter), _ptr(b_e),
+                                             _ptr(b_o), _ptr(x_e), _ptr(x_o), ctypes.byref(it), ctypes.byref(res)),
+                "oracle_stag_solve_full")
+    return dict(x_e=x_e, x_o=x_o, iters=it.value, true_residual=res.value, status=rc)

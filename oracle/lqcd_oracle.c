@@ -508,3 +508,73 @@ done:
     op_free(&op);
     return status;
 }
+
+/* ------------------------------------------------ full-system staggered solve */
+
+/* M = m + D on a full-lattice staggered vector given as its even and odd halves
+ * ("M = m + D, M^+ = m - D"): out_e = m in_e + D_eo in_o,
+ * out_o = m in_o + D_oe in_e. */
+int oracle_stag_M(const int *L, const double *u, double mass, const double *in_e, const double *in_o, double *out_e,
+                  double *out_o)
+{
+    geom_t G;
+    if (geom_init(&G, L)) return -1;
+    const long n = 3 * G.Vh;
+    const cd *ie = (const cd *)in_e, *io = (const cd *)in_o;
+    cd *oe = (cd *)out_e, *oo = (cd *)out_o;
+    stag_dslash(&G, (const cd *)u, 0, io, oe); /* D_eo in_o */
+    stag_dslash(&G, (const cd *)u, 1, ie, oo); /* D_oe in_e */
+    for (long i = 0; i < n; ++i) {
+        oe[i] = mass * ie[i] + oe[i];
+        oo[i] = mass * io[i] + oo[i];
+    }
+    return 0;
+}
+
+/* Solve M x = b on the full lattice, the way the hybrid molecular dynamics needs it
+ * (the paper's congrad has two outputs, copyout(x,y)).
+ * Written out in even/odd blocks, M x = b reads
+ *     m x_e + D_eo x_o = b_e,      m x_o + D_oe x_e = b_o,
+ * so   x_o = (b_o - D_oe x_e)/m   and   (m^2 - D_eo D_oe) x_e = m b_e - D_eo b_o.
+ * Steps, in this order:
+ *   1. b' = m b_e - D_eo b_o                      (source preparation)
+ *   2. CG on A x_e = b', A = m^2 - D_eo D_oe      (oracle_cg above, tol relative to |b'|)
+ *   3. x_o = (b_o - D_oe x_e)/m                   (reconstruction)
+ *   4. true_res = |b - M x| / |b| over the full lattice, with M applied afresh
+ * Returns the CG's status (0 converged, 1 maxiter); mass = 0 is an error (-2).
+ * b = 0 gives x = 0, iters = 0, true_res = 0. */
+int oracle_stag_solve_full(const int *L, const double *u_, double mass, double tol, int maxiter, const double *b_e_,
+                           const double *b_o_, double *x_e_, double *x_o_, int *iters, double *true_res)
+{
+    geom_t G;
+    if (geom_init(&G, L)) return -1;
+    if (mass == 0.0) return -2;
+    const long n = 3 * G.Vh;
+    const cd *u = (const cd *)u_, *be = (const cd *)b_e_, *bo = (const cd *)b_o_;
+    cd *xe = (cd *)x_e_, *xo = (cd *)x_o_;
+    cd *bp = malloc(sizeof(cd) * n), *t = malloc(sizeof(cd) * n), *me = malloc(sizeof(cd) * n), *mo = malloc(sizeof(cd) * n);
+    if (!bp || !t || !me || !mo) return -3;
+    /* 1 */
+    stag_dslash(&G, u, 0, bo, t);
+    for (long i = 0; i < n; ++i) bp[i] = mass * be[i] - t[i];
+    /* 2 */
+    double cg_res = 0.0;
+    const int status = oracle_cg(L, ORACLE_STAGGERED, u_, mass, tol, maxiter, (const double *)bp, x_e_, iters, &cg_res, NULL);
+    if (status < 0) return status;
+    /* 3 */
+    stag_dslash(&G, u, 1, xe, t);
+    for (long i = 0; i < n; ++i) xo[i] = (bo[i] - t[i]) / mass;
+    /* 4 */
+    oracle_stag_M(L, u_, mass, x_e_, x_o_, (double *)me, (double *)mo);
+    for (long i = 0; i < n; ++i) {
+        me[i] = be[i] - me[i];
+        mo[i] = bo[i] - mo[i];
+    }
+    const double bb = dot_re(be, be, n) + dot_re(bo, bo, n);
+    *true_res = bb > 0.0 ? sqrt((dot_re(me, me, n) + dot_re(mo, mo, n)) / bb) : 0.0;
+    free(bp);
+    free(t);
+    free(me);
+    free(mo);
+    return status;
+}
