@@ -129,6 +129,17 @@ int lqcd_apply_MdagM(lqcd_ctx *ctx, double mass_or_kappa, const double *in_dev, 
 int lqcd_cg_solve(lqcd_ctx *ctx, double mass_or_kappa, double tol, int maxiter, const double *b_dev, double *x_dev,
                   int *iters, double *true_residual);
 
+/* Full-system staggered solve M x = b, M = m + D, on the whole lattice (
+ * what the hybrid molecular dynamics around the paper's congrad needs, whose data region has two
+ * outputs, copyout(x,y)).  Even-odd reduction, every step in the CUDA kernels:
+ *   b' = m b_e - D_eo b_o;   CG on (m^2 - D_eo D_oe) x_e = b' (tol relative to |b'|, as lqcd_cg_solve);
+ *   x_o = (b_o - D_oe x_e)/m;   *true_residual = |b - M x| / |b| over both parities, M applied afresh.
+ * The four vectors are staggered half-lattice vectors [3][Vh] (even / odd sites); none may alias.
+ * *iters = CG iterations.  mass = 0 and a Wilson context are LQCD_EARG.  b = 0 gives x = 0. */
+int lqcd_stag_solve_full(lqcd_ctx *ctx, double mass, double tol, int maxiter, const double *b_even_dev,
+                         const double *b_odd_dev, double *x_even_dev, double *x_odd_dev, int *iters,
+                         double *true_residual);
+
 /* The paper's congrad with its data region (copyin(u,r) ... copyout(x)):
  * HOST buffers in the canonical layouts (pinned memory makes the copies asynchronous).
  * Copies u and b to the device, converts the gauge field, solves, copies x back. */

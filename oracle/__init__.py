@@ -57,6 +57,8 @@ def lib():
         L.oracle_cg.argtypes = [P, ctypes.c_int, P, ctypes.c_double, ctypes.c_double, ctypes.c_int, P, P, P, P, P]
         L.oracle_stag_M.argtypes = [P, P, ctypes.c_double, P, P, P, P]
         L.oracle_stag_solve_full.argtypes = [P, P, ctypes.c_double, ctypes.c_double, ctypes.c_int, P, P, P, P, P, P]
+        L.oracle_stag_dslash_f32.argtypes = [P, P, ctypes.c_int, P, P]
+        L.oracle_cg_mixed.argtypes = [P, P, ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_int, P, P, P, P, P, P]
         L.oracle_num_threads.restype = ctypes.c_int
         L.oracle_set_threads.argtypes = [ctypes.c_int]
         _lib = L
@@ -209,3 +211,33 @@ def stag_solve_full(dims, u, mass, tol, maxiter, b_e, b_o):
                                              _ptr(b_o), _ptr(x_e), _ptr(x_o), ctypes.byref(it), ctypes.byref(res)),
                 "oracle_stag_solve_full")
     return dict(x_e=x_e, x_o=x_o, iters=it.value, true_residual=res.value, status=rc)
+
+
+def stag_dslash_f32(dims, u, out_parity, vin):
+    """The staggered hopping term evaluated in fp32 on fl32(u), fl32(vin); returned widened to complex128."""
+    d = _dims(dims)
+    u = _c(u, np.complex128)
+    vin = _c(vin, np.complex128)
+    assert vin.shape == _vec_shape(dims, STAGGERED)
+    out = np.empty_like(vin)
+    _check(lib().oracle_stag_dslash_f32(_ptr(d), _ptr(u), int(out_parity), _ptr(vin), _ptr(out)), "oracle_stag_dslash_f32")
+    return out
+
+
+def cg_mixed(dims, u, mass, tol, maxiter, b, delta=0.1, history=False):
+    """Mixed-precision CG with reliable updates: dict(x, iters, updates, true_residual, status[, rr_history])."""
+    d = _dims(dims)
+    u = _c(u, np.complex128)
+    b = _c(b, np.complex128)
+    assert b.shape == _vec_shape(dims, STAGGERED)
+    x = np.empty_like(b)
+    it, nu = ctypes.c_int(0), ctypes.c_int(0)
+    res = ctypes.c_double(0.0)
+    hist = np.zeros(maxiter + 1, np.float64) if history else None
+    rc = _check(lib().oracle_cg_mixed(_ptr(d), _ptr(u), float(mass), float(tol), float(delta), int(maxiter), _ptr(b),
+                                      _ptr(x), ctypes.byref(it), ctypes.byref(nu), ctypes.byref(res),
+                                      _ptr(hist) if history else None), "oracle_cg_mixed")
+    out = dict(x=x, iters=it.value, updates=nu.value, true_residual=res.value, status=rc)
+    if history:
+        out["rr_history"] = hist[: it.value + 1]
+    return out

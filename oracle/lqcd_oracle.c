@@ -578,3 +578,223 @@ int oracle_stag_solve_full(const int *L, const double *u_, double mass, double t
     free(mo);
     return status;
 }
+
+/* ------------------------------------------- mixed-precision CG (fp32 inner) */
+
+/* the technique of the paper's reference [2] (Clark et al.,
+ * "Solving Lattice QCD systems of equations using mixed precision solvers on GPUs"): the CG
+ * iteration runs on fp32 copies of the links and vectors ("sloppy" precision) and is tied to the
+ * fp64 problem by RELIABLE UPDATES: whenever the iterated residual has dropped by the factor
+ * delta below the largest residual seen since the last update (or claims convergence), the
+ * partial solution is added to the fp64 solution, the residual is recomputed in fp64 from its
+ * definition b - A x, and the iteration continues from it keeping its search direction.
+ *
+ * What is fp32 and what is fp64 (DESIGN.md "Mixed precision" states the same contract):
+ *   - links uf = fl32(u), vectors xs, rs, ps, ts stored in fp32;
+ *   - the hopping term D^ is evaluated in fp32 arithmetic (stag_site_f below);
+ *   - every inner product is accumulated in fp64 from the fp32 values;
+ *   - the vector updates are evaluated in fp64 from the fp32 values and rounded on store;
+ *   - the scalars alpha, beta, <r,r>, the update test and the exit test are fp64;
+ *   - the reliable update (x, b - A x, its norm) is entirely fp64 with the fp64 operator. */
+typedef float complex cf;
+
+/* stag_site in fp32 arithmetic: same sum, same order. */
+static void stag_site_f(const geom_t *G, const cf *u, int parity, long e, const cf *in, cf out[3])
+{
+    int x[4];
+    site_coords(G, parity, e, x);
+    const long g = parity * G->Vh + e;
+    const long other = (1 - parity) * G->Vh;
+    cf acc[3] = { 0, 0, 0 };
+    for (int mu = 0; mu < 4; ++mu) {
+        const float eta = (float)eta_phase(x, mu);
+        {
+            const long ef = neighbour(G, x, mu, +1) - other;
+            const cf *U = u + (g * 4 + mu) * 9;
+            const float sgn = eta * (float)bc_forward(G, x, mu);
+            for (int a = 0; a < 3; ++a) {
+                cf s = 0;
+                for (int b = 0; b < 3; ++b) s += U[a * 3 + b] * in[b * G->Vh + ef];
+                acc[a] += sgn * s;
+            }
+        }
+        {
+            const long gb = neighbour(G, x, mu, -1);
+            const long eb = gb - other;
+            const cf *W = u + (gb * 4 + mu) * 9;
+            const float sgn = eta * (float)bc_backward(G, x, mu);
+            for (int a = 0; a < 3; ++a) {
+                cf s = 0;
+                for (int b = 0; b < 3; ++b) s += conjf(W[b * 3 + a]) * in[b * G->Vh + eb];
+                acc[a] -= sgn * s;
+            }
+        }
+    }
+    for (int a = 0; a < 3; ++a) out[a] = 0.5f * acc[a];
+}
+
+static void stag_dslash_f(const geom_t *G, const cf *u, int out_parity, const cf *in, cf *out)
+{
+#pragma omp parallel for schedule(static)
+    for (long e = 0; e < G->Vh; ++e) {
+        cf r[3];
+        stag_site_f(G, u, out_parity, e, in, r);
+        for (int a = 0; a < 3; ++a) out[a * G->Vh + e] = r[a];
+    }
+}
+
+/* Re<a,b> of fp32 vectors accumulated in fp64, fixed blocks as dot_re. */
+static double dot_re_f(const cf *a, const cf *b, long n)
+{
+    const long nb = (n + DOT_BLOCK - 1) / DOT_BLOCK;
+    double *part = malloc(sizeof(double) * (nb > 0 ? nb : 1));
+#pragma omp parallel for schedule(static)
+    for (long k = 0; k < nb; ++k) {
+        const long lo = k * DOT_BLOCK, hi = lo + DOT_BLOCK < n ? lo + DOT_BLOCK : n;
+        double s = 0.0;
+        for (long i = lo; i < hi; ++i)
+            s += (double)crealf(a[i]) * (double)crealf(b[i]) + (double)cimagf(a[i]) * (double)cimagf(b[i]);
+        part[k] = s;
+    }
+    double s = 0.0;
+    for (long k = 0; k < nb; ++k) s += part[k];
+    free(part);
+    return s;
+}
+
+/* The fp32 hopping term through the C interface (for its own pin against the fp64 one). */
+int oracle_stag_dslash_f32(const int *L, const double *u_, int out_parity, const double *in_, double *out_)
+{
+    geom_t G;
+    if (geom_init(&G, L)) return -1;
+    if (out_parity != 0 && out_parity != 1) return -2;
+    const long n = 3 * G.Vh, nu = G.V * 36;
+    const cd *u = (const cd *)u_, *in = (const cd *)in_;
+    cd *out = (cd *)out_;
+    cf *uf = malloc(sizeof(cf) * nu), *inf = malloc(sizeof(cf) * n), *of = malloc(sizeof(cf) * n);
+    if (!uf || !inf || !of) return -3;
+    for (long i = 0; i < nu; ++i) uf[i] = (cf)u[i];
+    for (long i = 0; i < n; ++i) inf[i] = (cf)in[i];
+    stag_dslash_f(&G, uf, out_parity, inf, of);
+    for (long i = 0; i < n; ++i) out[i] = (cd)of[i];
+    free(uf);
+    free(inf);
+    free(of);
+    return 0;
+}
+
+/* Mixed-precision conjugate gradient with reliable updates on A x = b, A = m^2 - D_eo D_oe
+ * (staggered, even sites).  Step by step (k counts applications of the fp32 operator):
+ *
+ *   x = 0 (fp64); bb = <b,b>; rr = bb; rs = ps = fl32(b); xs = 0; rmax = sqrt(rr)
+ *   for k = 1..maxiter:
+ *       ts = D^_oe ps;  qs = D^_eo ts                              (fp32 hopping terms)
+ *       alpha = rr / (m^2 <ps,ps> + <ts,ts>)                       (<p,Ap> from norms)
+ *       xs = fl32(xs + alpha ps);  rs = fl32(rs - alpha (m^2 ps - qs));  rr' = <rs,rs>
+ *       update = sqrt(rr') < delta*rmax  or  rr' <= tol^2 bb;      rmax = max(rmax, sqrt(rr'))
+ *       if update:                                                  (reliable update, all fp64)
+ *           x += xs; xs = 0;  r = b - A x;  rr' = <r,r>;  rs = fl32(r);  rmax = sqrt(rr')
+ *           if rr' <= tol^2 bb: converged, stop
+ *       beta = rr'/rr;  ps = fl32(rs + beta ps);  rr = rr'
+ *   if not converged: x += xs
+ *   true_res = |b - A x| / |b| with a fresh fp64 A
+ *
+ * So convergence is only ever declared on a residual computed in fp64 from its definition.
+ * Returns 0 converged / 1 maxiter; *nupdates = number of reliable updates; rr_hist[k] = rr' after
+ * iteration k (the fp64 value where an update took place). */
+int oracle_cg_mixed(const int *L, const double *u_, double mass, double tol, double delta, int maxiter,
+                    const double *b_, double *x_, int *iters, int *nupdates, double *true_res, double *rr_hist)
+{
+    op_t op;
+    int rc = op_init(&op, L, ORACLE_STAGGERED, (const cd *)u_, mass);
+    if (rc) return rc;
+    if (!(delta > 0.0 && delta < 1.0)) return -2;
+    const geom_t *G = &op.G;
+    const long n = op.n, nu = G->V * 36;
+    const double m2 = mass * mass;
+    const cd *b = (const cd *)b_, *u = (const cd *)u_;
+    cd *x = (cd *)x_;
+    cd *r = malloc(sizeof(cd) * n);
+    cf *uf = malloc(sizeof(cf) * nu), *xs = malloc(sizeof(cf) * n), *rs = malloc(sizeof(cf) * n);
+    cf *ps = malloc(sizeof(cf) * n), *ts = malloc(sizeof(cf) * n), *qs = malloc(sizeof(cf) * n);
+    if (!r || !uf || !xs || !rs || !ps || !ts || !qs) return -3;
+    for (long i = 0; i < nu; ++i) uf[i] = (cf)u[i];
+    for (long i = 0; i < n; ++i) {
+        x[i] = 0;
+        xs[i] = 0;
+        rs[i] = (cf)b[i];
+        ps[i] = rs[i];
+    }
+    double rr = dot_re(b, b, n);
+    const double bb = rr;
+    double rmax = sqrt(rr);
+    int status = 1, k = 0, nupd = 0;
+    if (rr_hist) rr_hist[0] = rr;
+    if (bb == 0.0) {
+        *iters = 0;
+        *nupdates = 0;
+        *true_res = 0.0;
+        status = 0;
+        goto done;
+    }
+    for (k = 1; k <= maxiter; ++k) {
+        stag_dslash_f(G, uf, 1, ps, ts);
+        stag_dslash_f(G, uf, 0, ts, qs);
+        const double alpha = rr / (m2 * dot_re_f(ps, ps, n) + dot_re_f(ts, ts, n));
+#pragma omp parallel for schedule(static)
+        for (long i = 0; i < n; ++i) {
+            const cd pv = (cd)ps[i];
+            const cd ap = m2 * pv - (cd)qs[i];
+            xs[i] = (cf)((cd)xs[i] + alpha * pv);
+            rs[i] = (cf)((cd)rs[i] - alpha * ap);
+        }
+        double rr_new = dot_re_f(rs, rs, n);
+        const double rn = sqrt(rr_new);
+        const int update = (rn < delta * rmax) || (rr_new <= tol * tol * bb);
+        if (rn > rmax) rmax = rn;
+        if (update) {
+#pragma omp parallel for schedule(static)
+            for (long i = 0; i < n; ++i) {
+                x[i] += (cd)xs[i];
+                xs[i] = 0;
+            }
+            apply_A(&op, x, r);
+#pragma omp parallel for schedule(static)
+            for (long i = 0; i < n; ++i) {
+                r[i] = b[i] - r[i];
+                rs[i] = (cf)r[i];
+            }
+            rr_new = dot_re(r, r, n);
+            rmax = sqrt(rr_new);
+            ++nupd;
+        }
+        if (rr_hist) rr_hist[k] = rr_new;
+        if (update && rr_new <= tol * tol * bb) {
+            status = 0;
+            break;
+        }
+        const double beta = rr_new / rr;
+#pragma omp parallel for schedule(static)
+        for (long i = 0; i < n; ++i) ps[i] = (cf)((cd)rs[i] + beta * (cd)ps[i]);
+        rr = rr_new;
+    }
+    *iters = status == 0 ? k : maxiter;
+    *nupdates = nupd;
+    if (status != 0) {
+        for (long i = 0; i < n; ++i) x[i] += (cd)xs[i];
+    }
+    apply_A(&op, x, r);
+#pragma omp parallel for schedule(static)
+    for (long i = 0; i < n; ++i) r[i] = b[i] - r[i];
+    *true_res = sqrt(dot_re(r, r, n) / bb);
+done:
+    free(r);
+    free(uf);
+    free(xs);
+    free(rs);
+    free(ps);
+    free(ts);
+    free(qs);
+    op_free(&op);
+    return status;
+}

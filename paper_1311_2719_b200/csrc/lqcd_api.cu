@@ -256,6 +256,90 @@ int ensure_host(lqcd_ctx* ctx)
     return LQCD_OK;
 }
 
+// Init (S6) and the iteration loop (S1-S5) of the conjugate gradient on A x = b.  On return the
+// stream is idle and ctx->h_sc[0] holds the final scalars (iter, rr_new, thresh, bb).
+int cg_run(lqcd_ctx* ctx, double mass_or_kappa, double tol, int maxiter, const cplx* b, cplx* x)
+{
+    int rc;
+    // S6: p = r = b, x = 0, rr = bb = pp = |b|^2
+    cg_init_kernel<kVecBlock><<<vec_grid(ctx), kVecBlock, 0, ctx->stream>>>(b, x, ctx->r(), ctx->p(), ctx->nvec, ctx->sc(),
+                                                                           ctx->rs(), ctx->hist(), tol, maxiter);
+    LQCD_LAUNCH_CHECK();
+
+    CgScalars* h = ctx->h_sc;
+    if (ctx->cg_mode == LQCD_CG_SYNC) {
+        // The paper's loop: one scalar comes back per iteration, the exit test runs on the host
+        // (PAPER.md:75-76, :91-93, :100).
+        rc = read_scalars(ctx, 0);
+        if (rc) return rc;
+        LQCD_CUDA(cudaEventSynchronize(ctx->ev[0]));
+        while (!h[0].done) {
+            rc = cg_iteration_kernels(ctx, mass_or_kappa, x);
+            if (rc) return rc;
+            rc = read_scalars(ctx, 0);
+            if (rc) return rc;
+            LQCD_CUDA(cudaEventSynchronize(ctx->ev[0]));
+            if (h[0].done) break;
+            rc = cg_pupdate(ctx);
+            if (rc) return rc;
+        }
+    } else {
+        // Same kernels, same order; batches of `check_every` iterations are enqueued while the
+        // previous batch's scalars are still on their way to the host.  Once the device sets
+        // `done`, every later kernel returns at once, so x, r and the iteration count are exactly
+        // those of the synchronous loop.
+        const int batch = ctx->check_every;
+        // LQCD_CG_GRAPH: the batch is captured once and replayed with one graph launch instead of
+        // 3*batch kernel launches (launch-bound small lattices).  The legacy default stream cannot
+        // be captured; there the batch is enqueued kernel by kernel as in LQCD_CG_ASYNC.
+        GraphHolder gh;
+        if (ctx->cg_mode == LQCD_CG_GRAPH && ctx->stream != nullptr && maxiter > 0) {
+            const long long counted = ctx->launches;
+            LQCD_CUDA(cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal));
+            rc = enqueue_batch(ctx, mass_or_kappa, x, batch);
+            cudaError_t ce = cudaStreamEndCapture(ctx->stream, &gh.graph);
+            if (rc) return rc;
+            LQCD_CUDA(ce);
+            LQCD_CUDA(cudaGraphInstantiate(&gh.exec, gh.graph, 0));
+            ctx->launches = counted;  // capturing launched nothing
+        }
+        int slot = 0;
+        bool pending[2] = { false, false };
+        bool finished = false;
+        long long enqueued = 0;
+        while (!finished) {
+            if (enqueued < (long long)maxiter) {
+                if (gh.exec) {
+                    LQCD_CUDA(cudaGraphLaunch(gh.exec, ctx->stream));
+                    ctx->launches += 3LL * batch;
+                } else {
+                    rc = enqueue_batch(ctx, mass_or_kappa, x, batch);
+                    if (rc) return rc;
+                }
+                enqueued += batch;
+            }
+            rc = read_scalars(ctx, slot);
+            if (rc) return rc;
+            pending[slot] = true;
+            const int other = slot ^ 1;
+            if (pending[other]) {
+                LQCD_CUDA(cudaEventSynchronize(ctx->ev[other]));
+                pending[other] = false;
+                if (h[other].done) finished = true;
+            }
+            slot = other;
+        }
+        // drain: the newest snapshot has the final values
+        LQCD_CUDA(cudaStreamSynchronize(ctx->stream));
+        rc = read_scalars(ctx, 0);
+        if (rc) return rc;
+        LQCD_CUDA(cudaEventSynchronize(ctx->ev[0]));
+    }
+
+    ctx->last_iters = h[0].iter;
+    return LQCD_OK;
+}
+
 }  // namespace
 
 // =========================================================================== C-ABI
@@ -433,6 +517,7 @@ int lqcd_apply_MdagM(lqcd_ctx* ctx, double mass_or_kappa, const double* in_dev, 
     return launch_wilson<WE_M, true>(ctx, wilson_args(ctx, 0, ctx->t(), (cplx*)out_dev, mass_or_kappa));
 }
 
+
 int lqcd_cg_solve(lqcd_ctx* ctx, double mass_or_kappa, double tol, int maxiter, const double* b_dev, double* x_dev,
                   int* iters, double* true_residual)
 {
@@ -443,81 +528,9 @@ int lqcd_cg_solve(lqcd_ctx* ctx, double mass_or_kappa, double tol, int maxiter, 
     if (!(tol >= 0.0) || maxiter < 0) return fail(ctx, LQCD_EARG, "tol must be >= 0 and maxiter >= 0");
     const cplx* b = (const cplx*)b_dev;
     cplx* x = (cplx*)x_dev;
-
-    // S6: p = r = b, x = 0, rr = bb = pp = |b|^2
-    cg_init_kernel<kVecBlock><<<vec_grid(ctx), kVecBlock, 0, ctx->stream>>>(b, x, ctx->r(), ctx->p(), ctx->nvec, ctx->sc(),
-                                                                           ctx->rs(), ctx->hist(), tol, maxiter);
-    LQCD_LAUNCH_CHECK();
-
     CgScalars* h = ctx->h_sc;
-    if (ctx->cg_mode == LQCD_CG_SYNC) {
-        // The paper's loop: one scalar comes back per iteration, the exit test runs on the host
-        // (PAPER.md:75-76, :91-93, :100).
-        rc = read_scalars(ctx, 0);
-        if (rc) return rc;
-        LQCD_CUDA(cudaEventSynchronize(ctx->ev[0]));
-        while (!h[0].done) {
-            rc = cg_iteration_kernels(ctx, mass_or_kappa, x);
-            if (rc) return rc;
-            rc = read_scalars(ctx, 0);
-            if (rc) return rc;
-            LQCD_CUDA(cudaEventSynchronize(ctx->ev[0]));
-            if (h[0].done) break;
-            rc = cg_pupdate(ctx);
-            if (rc) return rc;
-        }
-    } else {
-        // Same kernels, same order; batches of `check_every` iterations are enqueued while the
-        // previous batch's scalars are still on their way to the host.  Once the device sets
-        // `done`, every later kernel returns at once, so x, r and the iteration count are exactly
-        // those of the synchronous loop.
-        const int batch = ctx->check_every;
-        // LQCD_CG_GRAPH: the batch is captured once and replayed with one graph launch instead of
-        // 3*batch kernel launches (launch-bound small lattices).  The legacy default stream cannot
-        // be captured; there the batch is enqueued kernel by kernel as in LQCD_CG_ASYNC.
-        GraphHolder gh;
-        if (ctx->cg_mode == LQCD_CG_GRAPH && ctx->stream != nullptr && maxiter > 0) {
-            const long long counted = ctx->launches;
-            LQCD_CUDA(cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal));
-            rc = enqueue_batch(ctx, mass_or_kappa, x, batch);
-            cudaError_t ce = cudaStreamEndCapture(ctx->stream, &gh.graph);
-            if (rc) return rc;
-            LQCD_CUDA(ce);
-            LQCD_CUDA(cudaGraphInstantiate(&gh.exec, gh.graph, 0));
-            ctx->launches = counted;  // capturing launched nothing
-        }
-        int slot = 0;
-        bool pending[2] = { false, false };
-        bool finished = false;
-        long long enqueued = 0;
-        while (!finished) {
-            if (enqueued < (long long)maxiter) {
-                if (gh.exec) {
-                    LQCD_CUDA(cudaGraphLaunch(gh.exec, ctx->stream));
-                    ctx->launches += 3LL * batch;
-                } else {
-                    rc = enqueue_batch(ctx, mass_or_kappa, x, batch);
-                    if (rc) return rc;
-                }
-                enqueued += batch;
-            }
-            rc = read_scalars(ctx, slot);
-            if (rc) return rc;
-            pending[slot] = true;
-            const int other = slot ^ 1;
-            if (pending[other]) {
-                LQCD_CUDA(cudaEventSynchronize(ctx->ev[other]));
-                pending[other] = false;
-                if (h[other].done) finished = true;
-            }
-            slot = other;
-        }
-        // drain: the newest snapshot has the final values
-        LQCD_CUDA(cudaStreamSynchronize(ctx->stream));
-        rc = read_scalars(ctx, 0);
-        if (rc) return rc;
-        LQCD_CUDA(cudaEventSynchronize(ctx->ev[0]));
-    }
+    rc = cg_run(ctx, mass_or_kappa, tol, maxiter, b, x);
+    if (rc) return rc;
 
     // S7: true residual |b - A x| / |b| with a fresh application of A
     rc = op_first(ctx, mass_or_kappa, x, false);
@@ -539,9 +552,67 @@ int lqcd_cg_solve(lqcd_ctx* ctx, double mass_or_kappa, double tol, int maxiter, 
     LQCD_CUDA(cudaEventSynchronize(ctx->ev[0]));
 
     *iters = h[0].iter;
-    ctx->last_iters = h[0].iter;
     *true_residual = h[0].bb > 0.0 ? sqrt(h[0].res2 / h[0].bb) : 0.0;
     const bool converged = h[0].rr_new <= h[0].thresh;
+    return converged ? LQCD_OK : LQCD_MAXITER;
+}
+
+int lqcd_stag_solve_full(lqcd_ctx* ctx, double mass, double tol, int maxiter, const double* b_even_dev,
+                         const double* b_odd_dev, double* x_even_dev, double* x_odd_dev, int* iters,
+                         double* true_residual)
+{
+    int rc = check_ready(ctx, true);
+    if (rc) return rc;
+    if (ctx->fermion != LQCD_STAGGERED) return fail(ctx, LQCD_EARG, "lqcd_stag_solve_full needs a staggered context");
+    if (!b_even_dev || !b_odd_dev || !x_even_dev || !x_odd_dev || !iters || !true_residual)
+        return fail(ctx, LQCD_EARG, "null pointer argument");
+    if (x_even_dev == x_odd_dev || b_even_dev == x_even_dev || b_even_dev == x_odd_dev || b_odd_dev == x_even_dev ||
+        b_odd_dev == x_odd_dev)
+        return fail(ctx, LQCD_EARG, "b and x vectors must not alias");
+    if (!(tol >= 0.0) || maxiter < 0) return fail(ctx, LQCD_EARG, "tol must be >= 0 and maxiter >= 0");
+    if (mass == 0.0 || !(mass == mass)) return fail(ctx, LQCD_EARG, "mass must be non-zero (x_o = (b_o - D_oe x_e)/m)");
+    const cplx *be = (const cplx*)b_even_dev, *bo = (const cplx*)b_odd_dev;
+    cplx *xe = (cplx*)x_even_dev, *xo = (cplx*)x_odd_dev;
+    cplx* bp = (cplx*)(ctx->ws + ctx->off_stage_b);  // b' lives in the staging area (idle during device-pointer calls)
+    CgScalars* h = ctx->h_sc;
+
+    // 1. source preparation  b' = m b_e - D_eo b_o
+    StagArgsD a = stag_args(ctx, LQCD_EVEN, bo, bp);
+    a.m2 = mass;
+    a.p = be;
+    rc = launch_stag<SE_PREP>(ctx, a);
+    if (rc) return rc;
+    // 2. CG on (m^2 - D_eo D_oe) x_e = b'
+    rc = cg_run(ctx, mass, tol, maxiter, bp, xe);
+    if (rc) return rc;
+    const int cg_iters = h[0].iter;
+    const bool converged = h[0].rr_new <= h[0].thresh;
+    // 3. reconstruction  x_o = (b_o - D_oe x_e)/m
+    a = stag_args(ctx, LQCD_ODD, xe, xo);
+    a.m2 = mass;
+    a.p = bo;
+    rc = launch_stag<SE_RECON>(ctx, a);
+    if (rc) return rc;
+    // 4. |b - M x|^2 and |b|^2 over both parities with M = m + D applied afresh
+    a = stag_args(ctx, LQCD_EVEN, xo, nullptr);
+    a.m2 = mass;
+    a.p = xe;
+    a.b = be;
+    a.flag = 0;
+    rc = launch_stag<SE_RESIDUAL_M>(ctx, a);
+    if (rc) return rc;
+    a = stag_args(ctx, LQCD_ODD, xe, nullptr);
+    a.m2 = mass;
+    a.p = xo;
+    a.b = bo;
+    a.flag = 1;
+    rc = launch_stag<SE_RESIDUAL_M>(ctx, a);
+    if (rc) return rc;
+    rc = read_scalars(ctx, 0);
+    if (rc) return rc;
+    LQCD_CUDA(cudaEventSynchronize(ctx->ev[0]));
+    *iters = cg_iters;
+    *true_residual = h[0].aux > 0.0 ? sqrt(h[0].res2 / h[0].aux) : 0.0;
     return converged ? LQCD_OK : LQCD_MAXITER;
 }
 

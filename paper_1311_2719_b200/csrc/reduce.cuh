@@ -96,4 +96,36 @@ __device__ __forceinline__ void grid_sum(double local, const ReduceScratch& rs, 
     }
 }
 
+// The same for N sums at once (partials laid out [N][gridDim.x]); `fin(total[N])`.
+template <int BLOCK, int N, class Finalise>
+__device__ __forceinline__ void grid_sum_n(const double (&local)[N], const ReduceScratch& rs, Finalise fin)
+{
+    __shared__ bool is_last_n;
+    double s[N];
+#pragma unroll
+    for (int k = 0; k < N; ++k) s[k] = block_sum<BLOCK>(local[k]);
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int k = 0; k < N; ++k) rs.partials[(size_t)k * gridDim.x + blockIdx.x] = s[k];
+        __threadfence();
+        unsigned int t = atomicAdd(rs.ticket, 1u);
+        is_last_n = (t == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (is_last_n) {
+        __threadfence();
+        double total[N];
+#pragma unroll
+        for (int k = 0; k < N; ++k) {
+            double acc = 0.0;
+            for (unsigned int i = threadIdx.x; i < gridDim.x; i += BLOCK) acc += __ldcg(rs.partials + (size_t)k * gridDim.x + i);
+            total[k] = block_sum<BLOCK>(acc);
+        }
+        if (threadIdx.x == 0) {
+            *rs.ticket = 0u;
+            fin(total);
+        }
+    }
+}
+
 }  // namespace lqcd

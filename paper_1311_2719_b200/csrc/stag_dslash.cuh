@@ -23,7 +23,11 @@ enum StagEpilogue {
     SE_NORM = 1,      // out = D in, tt = |out|^2, alpha = rr/(m^2 pp + tt)     (S1 + S2)
     SE_MDAGM = 2,     // out = m^2 p - D in                                     (lqcd_apply_MdagM, 2nd hop)
     SE_CGUPDATE = 3,  // Ap = m^2 p - D in; x += alpha p; r -= alpha Ap; |r|^2  (S3), Ap never stored
-    SE_RESIDUAL = 4   // |b - (m^2 p - D in)|^2                                 (S7), nothing stored
+    SE_RESIDUAL = 4,  // |b - (m^2 p - D in)|^2                                 (S7), nothing stored
+    // full-system solve M x = b, M = m + D; `m2` carries the mass m here
+    SE_PREP = 5,      // out = m p - D in              source preparation  b' = m b_e - D_eo b_o
+    SE_RECON = 6,     // out = (p - D in)/m            reconstruction      x_o = (b_o - D_oe x_e)/m
+    SE_RESIDUAL_M = 7 // |b - (m p + D in)|^2 and |b|^2 of one parity, set (flag = 0) or added (flag = 1)
 };
 
 template <class C>
@@ -38,6 +42,7 @@ struct StagArgs {
     C* r;
     const C* b;
     double m2;
+    int flag;
     CgScalars* sc;
     ReduceScratch rs;
     double* hist;
@@ -83,11 +88,15 @@ __device__ __forceinline__ void stag_hop(const StagArgs<C>& a, const Site& s, C 
 
 // Epilogue arithmetic is done in fp64 whatever the storage type C (free for fp64, a handful of
 // converts per site for the fp32 inner iterations of the mixed-precision solver).
-// Minimum resident blocks per SM.  Two-row links: without a bound ptxas keeps both links of a hop
-// and their rebuilt rows live (128-138 registers, 3 blocks/SM: 6.2 TB/s); 4 blocks/SM caps it at
-// 128 and measured best on B200 (65.4 us at 32^4 = 6.9 TB/s; 5 -> 68 us, 6+ spills -> 100+ us).
+// Minimum resident blocks per SM (measured on B200 at 32^4, profiles/):
+// all nine entries: the plain Dslash runs at 93-94 us whatever the bound (252 registers at 1, 72 at
+// 7), but the kernels with a CG epilogue gain from occupancy because the epilogue's loads of p, r, x
+// are issued after the hops: 247 us per CG iteration at 1-2 blocks/SM, 239 at 4-5, 235 at 7.
+// Two-row links: without a bound ptxas keeps both links of a hop and their rebuilt rows live
+// (128-138 registers, 3 blocks/SM: 6.2 TB/s); 4 blocks/SM caps it at 128 and measured best
+// (65.4 us = 6.9 TB/s; 5 -> 68 us, 6+ spills -> 100+ us).
 #ifndef LQCD_STAG_MINB18
-#define LQCD_STAG_MINB18 1
+#define LQCD_STAG_MINB18 7
 #endif
 #ifndef LQCD_STAG_MINB12
 #define LQCD_STAG_MINB12 4
@@ -160,6 +169,35 @@ __global__ void __launch_bounds__(BLOCK, RECON == 12 ? LQCD_STAG_MINB12 : LQCD_S
         CgScalars* sc = a.sc;
         double* hist = a.hist;
         grid_sum<BLOCK>(local, a.rs, [sc, hist](double rr_new) { cg_after_update(sc, hist, rr_new); });
+    } else if (EPI == SE_PREP || EPI == SE_RECON) {
+        if (active) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const double2 pv = to_d(a.p[c * Vh + e]), q = to_d(acc[c]);
+                const double2 o = EPI == SE_PREP ? cmake(fma(a.m2, pv.x, -q.x), fma(a.m2, pv.y, -q.y))
+                                                 : cmake((pv.x - q.x) / a.m2, (pv.y - q.y) / a.m2);
+                st_vec(a.out + c * Vh + e, to_cplx(o, (C*)0));
+            }
+        }
+    } else if (EPI == SE_RESIDUAL_M) {
+        double local[2] = { 0.0, 0.0 };
+        if (active) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const size_t i = c * Vh + e;
+                const double2 xv = to_d(a.p[i]), bv = to_d(a.b[i]), q = to_d(acc[c]);
+                const double re = bv.x - fma(a.m2, xv.x, q.x);
+                const double im = bv.y - fma(a.m2, xv.y, q.y);
+                local[0] += fma(re, re, im * im);
+                local[1] += cnorm2(bv);
+            }
+        }
+        CgScalars* sc = a.sc;
+        const int add = a.flag;
+        grid_sum_n<BLOCK, 2>(local, a.rs, [sc, add](const double (&tot)[2]) {
+            sc->res2 = add ? sc->res2 + tot[0] : tot[0];
+            sc->aux = add ? sc->aux + tot[1] : tot[1];
+        });
     } else {  // SE_RESIDUAL
         double local = 0.0;
         if (active) {

@@ -68,6 +68,7 @@ def load_library():
     L.lqcd_dslash.argtypes = [P, I, P, P]
     L.lqcd_apply_MdagM.argtypes = [P, D, P, P]
     L.lqcd_cg_solve.argtypes = [P, D, D, I, P, P, ctypes.POINTER(I), ctypes.POINTER(D)]
+    L.lqcd_stag_solve_full.argtypes = [P, D, D, I, P, P, P, P, ctypes.POINTER(I), ctypes.POINTER(D)]
     L.lqcd_congrad_host.argtypes = [P, P, D, D, I, P, P, ctypes.POINTER(I), ctypes.POINTER(D)]
     L.lqcd_dslash_host.argtypes = [P, I, P, P]
     L.lqcd_cg_history.argtypes = [P, P, I]
@@ -224,6 +225,22 @@ class Lattice:
                                                  _cptr(x), ctypes.byref(it), ctypes.byref(res)))
         self._sync_out()
         return x, it.value, res.value, rc
+
+    def stag_solve_full(self, mass: float, tol: float, maxiter: int, b_even: torch.Tensor, b_odd: torch.Tensor,
+                        x_even: torch.Tensor | None = None, x_odd: torch.Tensor | None = None):
+        """M x = b on the full lattice (M = m + D): returns (x_even, x_odd, iters, true_residual, status)."""
+        self._vec(b_even, "b_even")
+        self._vec(b_odd, "b_odd")
+        x_even = torch.empty_like(b_even) if x_even is None else self._vec(x_even, "x_even")
+        x_odd = torch.empty_like(b_odd) if x_odd is None else self._vec(x_odd, "x_odd")
+        it = ctypes.c_int(0)
+        res = ctypes.c_double(0.0)
+        self._sync_in()
+        rc = self._check(self._lib.lqcd_stag_solve_full(self._ctx, float(mass), float(tol), int(maxiter), _cptr(b_even),
+                                                        _cptr(b_odd), _cptr(x_even), _cptr(x_odd), ctypes.byref(it),
+                                                        ctypes.byref(res)))
+        self._sync_out()
+        return x_even, x_odd, it.value, res.value, rc
 
     def congrad_host(self, u_host: torch.Tensor, mass_or_kappa: float, tol: float, maxiter: int, b_host: torch.Tensor,
                      x_host: torch.Tensor | None = None):
