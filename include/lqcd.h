@@ -129,6 +129,22 @@ int lqcd_apply_MdagM(lqcd_ctx *ctx, double mass_or_kappa, const double *in_dev, 
 int lqcd_cg_solve(lqcd_ctx *ctx, double mass_or_kappa, double tol, int maxiter, const double *b_dev, double *x_dev,
                   int *iters, double *true_residual);
 
+/* Mixed-precision conjugate gradient with reliable updates on the same system as lqcd_cg_solve
+ * (staggered contexts; the technique of the paper's reference [2],
+ * PAPER.md:151).  The iteration (S1-S5) runs on fp32 copies of the links and of x, r, p, t -- half
+ * the bytes per iteration -- and is tied to the fp64 problem by reliable updates: when the iterated
+ * |r| has fallen below delta times the largest |r| since the last update, or claims convergence,
+ * x_dev += xs in fp64, r = b - A x is recomputed in fp64 from its definition with the fp64 links,
+ * and the iteration resumes from fl32(r) keeping its search direction.  Convergence
+ * (<r,r> <= tol^2 <b,b>) is only ever declared on such an fp64 residual, so *true_residual <= tol
+ * holds as for lqcd_cg_solve.  fp32/fp64 split: hopping terms in fp32; inner products accumulated in
+ * fp64; vector updates evaluated in fp64 and rounded on store; all scalars and tests fp64.
+ * delta in (0,1), typically 0.1.  *iters = fp32 iterations, *reliable_updates = fp64 updates.
+ * Contract: the solution agrees with lqcd_cg_solve's within 2 tol |b| / (m^2 |x|);
+ * iteration counts are NOT comparable to +-2 (fp32 rounding changes the trajectory). */
+int lqcd_cg_solve_mixed(lqcd_ctx *ctx, double mass, double tol, int maxiter, double delta, const double *b_dev,
+                        double *x_dev, int *iters, int *reliable_updates, double *true_residual);
+
 /* Full-system staggered solve M x = b, M = m + D, on the whole lattice (
  * what the hybrid molecular dynamics around the paper's congrad needs, whose data region has two
  * outputs, copyout(x,y)).  Even-odd reduction, every step in the CUDA kernels:

@@ -34,26 +34,99 @@ __global__ void __launch_bounds__(BLOCK) cg_init_kernel(const cplx* __restrict__
         sc->iter = 0;
         sc->maxiter = maxiter;
         sc->done = (bb == 0.0 || maxiter <= 0) ? 1 : 0;  // b = 0: x = 0, iters = 0 (reading A11)
+        sc->pause = 0;
+        sc->nupd = 0;
         hist[0] = bb;
     });
 }
 
+// S6 of the mixed-precision solver: x = 0 (fp64), xs = 0, rs = ps = fl32(b),
+// rr = bb = <b,b> from the fp64 source, pp = <ps,ps> from the fp32 copy, rmax = |b|.
+template <int BLOCK>
+__global__ void __launch_bounds__(BLOCK) cg_init_mixed_kernel(const cplx* __restrict__ b, cplx* __restrict__ x,
+                                                              cplxf* __restrict__ xs, cplxf* __restrict__ rs,
+                                                              cplxf* __restrict__ ps, size_t n, CgScalars* sc,
+                                                              ReduceScratch rs_, double* hist, double tol, double delta,
+                                                              int maxiter)
+{
+    double local[2] = { 0.0, 0.0 };
+    for (size_t i = (size_t)blockIdx.x * BLOCK + threadIdx.x; i < n; i += (size_t)gridDim.x * BLOCK) {
+        const cplx v = b[i];
+        const cplxf vf = make_float2((float)v.x, (float)v.y);
+        x[i] = cmake(0.0, 0.0);
+        xs[i] = make_float2(0.f, 0.f);
+        rs[i] = vf;
+        ps[i] = vf;
+        local[0] += cnorm2(v);
+        local[1] += cnorm2(vf);
+    }
+    grid_sum_n<BLOCK, 2>(local, rs_, [sc, hist, tol, delta, maxiter](const double (&tot)[2]) {
+        const double bb = tot[0];
+        sc->rr = bb;
+        sc->rr_new = bb;
+        sc->bb = bb;
+        sc->pp = tot[1];
+        sc->tt = 0.0;
+        sc->alpha = 0.0;
+        sc->beta = 0.0;
+        sc->thresh = tol * tol * bb;
+        sc->res2 = 0.0;
+        sc->rmax = sqrt(bb);
+        sc->delta = delta;
+        sc->iter = 0;
+        sc->maxiter = maxiter;
+        sc->done = (bb == 0.0 || maxiter <= 0) ? 1 : 0;
+        sc->pause = 0;
+        sc->nupd = 0;
+        hist[0] = bb;
+    });
+}
+
+// Reliable update, first step: x += xs (fp64), xs = 0.  `only_if_paused` = 1 inside the iteration
+// (a stale launch must not touch anything); 0 for the final accumulation after the loop has ended.
+template <int BLOCK>
+__global__ void __launch_bounds__(BLOCK) mixed_accumulate_kernel(cplx* __restrict__ x, cplxf* __restrict__ xs, size_t n,
+                                                                 const CgScalars* sc, int only_if_paused)
+{
+    if (only_if_paused && !sc->pause) return;
+    for (size_t i = (size_t)blockIdx.x * BLOCK + threadIdx.x; i < n; i += (size_t)gridDim.x * BLOCK) {
+        const cplxf d = xs[i];
+        cplx v = x[i];
+        v.x += (double)d.x;
+        v.y += (double)d.y;
+        x[i] = v;
+        xs[i] = make_float2(0.f, 0.f);
+    }
+}
+
+// fp64 structure-of-arrays links -> fp32 copy of the same layout (built once per loaded gauge field).
+__global__ void gauge_narrow_kernel(const cplx* __restrict__ g64, cplxf* __restrict__ g32, size_t n)
+{
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const cplx v = g64[i];
+        g32[i] = make_float2((float)v.x, (float)v.y);
+    }
+}
+
 // S5 (PAPER.md:96 gives beta; the p-update itself fell off the truncated listing, reading A7):
 // p = r + beta p, pp = <p,p>.
-template <int BLOCK>
-__global__ void __launch_bounds__(BLOCK) cg_pupdate_kernel(const cplx* __restrict__ r, cplx* __restrict__ p, size_t n,
+// C = cplx (the fp64 path) or cplxf (the fp32 inner iteration: evaluated in fp64, rounded on store,
+// the norm taken of the stored value).
+template <int BLOCK, class C>
+__global__ void __launch_bounds__(BLOCK) cg_pupdate_kernel(const C* __restrict__ r, C* __restrict__ p, size_t n,
                                                            CgScalars* sc, ReduceScratch rs)
 {
-    if (sc->done) return;
+    if (sc->done | sc->pause) return;
     const double beta = sc->beta;
     double local = 0.0;
     for (size_t i = (size_t)blockIdx.x * BLOCK + threadIdx.x; i < n; i += (size_t)gridDim.x * BLOCK) {
-        const cplx rv = r[i];
-        cplx pv = p[i];
+        const double2 rv = to_d(r[i]);
+        double2 pv = to_d(p[i]);
         pv.x = fma(beta, pv.x, rv.x);
         pv.y = fma(beta, pv.y, rv.y);
-        p[i] = pv;
-        local += cnorm2(pv);
+        const C ps = to_cplx(pv, (C*)0);
+        p[i] = ps;
+        local += cnorm2(ps);
     }
     grid_sum<BLOCK>(local, rs, [sc](double pp) { sc->pp = pp; });
 }

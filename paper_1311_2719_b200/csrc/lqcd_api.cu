@@ -25,6 +25,7 @@ constexpr int kReorderTile = 64;
 constexpr size_t kAlign = 256;
 
 typedef StagArgs<cplx> StagArgsD;
+typedef StagArgs<cplxf> StagArgsF;
 
 size_t align_up(size_t n) { return (n + kAlign - 1) / kAlign * kAlign; }
 
@@ -38,12 +39,14 @@ struct lqcd_ctx {
     // workspace layout (byte offsets)
     size_t off_gauge, off_r, off_p, off_t, off_sc, off_ticket, off_partials, off_hist, off_stage;
     size_t off_stage_b, off_stage_x;  // inside the staging area, after the canonical gauge copy
+    size_t off_gauge_f, off_xf, off_rf, off_pf, off_tf;  // fp32 copies for the mixed-precision solver (staggered)
     size_t ws_needed;
     size_t max_blocks;
     // bound workspace
     char* ws;
     cudaStream_t stream;
     bool gauge_loaded;
+    bool gauge_f_ready;  // the fp32 link copy matches the loaded fp64 one
     // options
     int cg_mode;
     int check_every;
@@ -60,6 +63,11 @@ struct lqcd_ctx {
     cplx* r() const { return (cplx*)(ws + off_r); }
     cplx* p() const { return (cplx*)(ws + off_p); }
     cplx* t() const { return (cplx*)(ws + off_t); }
+    cplxf* gauge_f() const { return (cplxf*)(ws + off_gauge_f); }
+    cplxf* xf() const { return (cplxf*)(ws + off_xf); }
+    cplxf* rf() const { return (cplxf*)(ws + off_rf); }
+    cplxf* pf() const { return (cplxf*)(ws + off_pf); }
+    cplxf* tf() const { return (cplxf*)(ws + off_tf); }
     CgScalars* sc() const { return (CgScalars*)(ws + off_sc); }
     double* hist() const { return (double*)(ws + off_hist); }
     ReduceScratch rs() const
@@ -148,6 +156,34 @@ int launch_stag(lqcd_ctx* ctx, const StagArgsD& a)
     return LQCD_OK;
 }
 
+// fp32 instantiations: only the two kernels of the inner iteration of the mixed-precision solver
+StagArgsF stag_args_f(const lqcd_ctx* ctx, int parity, const cplxf* in, cplxf* out)
+{
+    StagArgsF a;
+    memset(&a, 0, sizeof a);
+    a.g = ctx->g;
+    a.parity = parity;
+    a.gauge = ctx->gauge_f();
+    a.in = in;
+    a.out = out;
+    a.sc = ctx->sc();
+    a.rs = ctx->rs();
+    a.hist = ctx->hist();
+    return a;
+}
+
+template <int EPI>
+int launch_stag_f(lqcd_ctx* ctx, const StagArgsF& a)
+{
+    const unsigned int grid = blocks_for(ctx->g.Vh, kStagBlock);
+    if (ctx->recon == 12)
+        stag_dslash_kernel<EPI, kStagBlock, 12, cplxf><<<grid, kStagBlock, 0, ctx->stream>>>(a);
+    else
+        stag_dslash_kernel<EPI, kStagBlock, 18, cplxf><<<grid, kStagBlock, 0, ctx->stream>>>(a);
+    LQCD_LAUNCH_CHECK();
+    return LQCD_OK;
+}
+
 // ---------------------------------------------------------------- Wilson launches
 WilsonArgs wilson_args(const lqcd_ctx* ctx, int parity, const cplx* in, cplx* out, double kappa)
 {
@@ -212,7 +248,7 @@ int cg_iteration_kernels(lqcd_ctx* ctx, double param, cplx* x)
 
 int cg_pupdate(lqcd_ctx* ctx)  // S5
 {
-    cg_pupdate_kernel<kVecBlock><<<vec_grid(ctx), kVecBlock, 0, ctx->stream>>>(ctx->r(), ctx->p(), ctx->nvec, ctx->sc(),
+    cg_pupdate_kernel<kVecBlock, cplx><<<vec_grid(ctx), kVecBlock, 0, ctx->stream>>>(ctx->r(), ctx->p(), ctx->nvec, ctx->sc(),
                                                                               ctx->rs());
     LQCD_LAUNCH_CHECK();
     return LQCD_OK;
@@ -340,6 +376,127 @@ int cg_run(lqcd_ctx* ctx, double mass_or_kappa, double tol, int maxiter, const c
     return LQCD_OK;
 }
 
+// ---------------------------------------------------------------- mixed precision
+int mixed_iteration_kernels(lqcd_ctx* ctx, double mass)  // S1 + S2, S3 on the fp32 copies
+{
+    StagArgsF a = stag_args_f(ctx, LQCD_ODD, ctx->pf(), ctx->tf());
+    a.m2 = mass * mass;
+    int rc = launch_stag_f<SE_NORM>(ctx, a);
+    if (rc) return rc;
+    a = stag_args_f(ctx, LQCD_EVEN, ctx->tf(), nullptr);
+    a.m2 = mass * mass;
+    a.p = ctx->pf();
+    a.x = ctx->xf();
+    a.r = ctx->rf();
+    return launch_stag_f<SE_CGUPDATE_MIXED>(ctx, a);
+}
+
+int mixed_pupdate(lqcd_ctx* ctx)  // S5 on the fp32 copies
+{
+    cg_pupdate_kernel<kVecBlock, cplxf><<<vec_grid(ctx), kVecBlock, 0, ctx->stream>>>(ctx->rf(), ctx->pf(), ctx->nvec,
+                                                                                      ctx->sc(), ctx->rs());
+    LQCD_LAUNCH_CHECK();
+    return LQCD_OK;
+}
+
+int mixed_batch(lqcd_ctx* ctx, double mass, int batch)
+{
+    for (int k = 0; k < batch; ++k) {
+        int rc = mixed_iteration_kernels(ctx, mass);
+        if (rc) return rc;
+        rc = mixed_pupdate(ctx);
+        if (rc) return rc;
+    }
+    return LQCD_OK;
+}
+
+// The reliable update, all fp64: x += xs, xs = 0; r = b - A x; rs = fl32(r); <r,r>, beta, exit test;
+// then the p-update the paused iteration was waiting for.  Enqueued by the host only after a
+// snapshot of the scalars showed `pause` with every earlier update completed.
+int mixed_reliable_update(lqcd_ctx* ctx, double mass, const cplx* b, cplx* x)
+{
+    mixed_accumulate_kernel<kVecBlock><<<vec_grid(ctx), kVecBlock, 0, ctx->stream>>>(x, ctx->xf(), ctx->nvec, ctx->sc(), 1);
+    LQCD_LAUNCH_CHECK();
+    int rc = launch_stag<SE_PLAIN>(ctx, stag_args(ctx, LQCD_ODD, x, ctx->t()));
+    if (rc) return rc;
+    StagArgsD a = stag_args(ctx, LQCD_EVEN, ctx->t(), nullptr);
+    a.m2 = mass * mass;
+    a.p = x;
+    a.b = b;
+    a.rf = ctx->rf();
+    rc = launch_stag<SE_RELIABLE>(ctx, a);
+    if (rc) return rc;
+    return mixed_pupdate(ctx);
+}
+
+int cg_run_mixed(lqcd_ctx* ctx, double mass, double tol, double delta, int maxiter, const cplx* b, cplx* x)
+{
+    int rc;
+    if (!ctx->gauge_f_ready) {
+        const size_t n = (size_t)ctx->g.V * 4 * (size_t)(ctx->recon / 2);
+        gauge_narrow_kernel<<<148 * 8, 256, 0, ctx->stream>>>(ctx->gauge(), ctx->gauge_f(), n);
+        LQCD_LAUNCH_CHECK();
+        ctx->gauge_f_ready = true;
+    }
+    cg_init_mixed_kernel<kVecBlock><<<vec_grid(ctx), kVecBlock, 0, ctx->stream>>>(
+        b, x, ctx->xf(), ctx->rf(), ctx->pf(), ctx->nvec, ctx->sc(), ctx->rs(), ctx->hist(), tol, delta, maxiter);
+    LQCD_LAUNCH_CHECK();
+
+    CgScalars* h = ctx->h_sc;
+    const bool sync = ctx->cg_mode == LQCD_CG_SYNC;
+    const int batch = sync ? 1 : ctx->check_every;
+    GraphHolder gh;
+    if (ctx->cg_mode == LQCD_CG_GRAPH && ctx->stream != nullptr && maxiter > 0) {
+        const long long counted = ctx->launches;
+        LQCD_CUDA(cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal));
+        rc = mixed_batch(ctx, mass, batch);
+        cudaError_t ce = cudaStreamEndCapture(ctx->stream, &gh.graph);
+        if (rc) return rc;
+        LQCD_CUDA(ce);
+        LQCD_CUDA(cudaGraphInstantiate(&gh.exec, gh.graph, 0));
+        ctx->launches = counted;
+    }
+    // As cg_run, with one more device-side state: `pause`.  Iterations enqueued after the device
+    // paused are no-ops, so the iterates do not depend on the batch size or on when the host notices.
+    int slot = 0, updates_enqueued = 0;
+    bool pending[2] = { false, false };
+    bool finished = maxiter <= 0;
+    while (!finished) {
+        if (gh.exec) {
+            LQCD_CUDA(cudaGraphLaunch(gh.exec, ctx->stream));
+            ctx->launches += 3LL * batch;
+        } else {
+            rc = mixed_batch(ctx, mass, batch);
+            if (rc) return rc;
+        }
+        rc = read_scalars(ctx, slot);
+        if (rc) return rc;
+        pending[slot] = true;
+        const int look = sync ? slot : slot ^ 1;
+        if (pending[look]) {
+            LQCD_CUDA(cudaEventSynchronize(ctx->ev[look]));
+            pending[look] = false;
+            if (h[look].done) {
+                finished = true;
+            } else if (h[look].pause && h[look].nupd == updates_enqueued) {
+                rc = mixed_reliable_update(ctx, mass, b, x);
+                if (rc) return rc;
+                ++updates_enqueued;
+            }
+        }
+        slot ^= 1;
+    }
+    // whatever the fp32 iteration still holds goes into x (nothing after a converged exit: xs = 0)
+    mixed_accumulate_kernel<kVecBlock><<<vec_grid(ctx), kVecBlock, 0, ctx->stream>>>(x, ctx->xf(), ctx->nvec, ctx->sc(), 0);
+    LQCD_LAUNCH_CHECK();
+    LQCD_CUDA(cudaStreamSynchronize(ctx->stream));
+    rc = read_scalars(ctx, 0);
+    if (rc) return rc;
+    LQCD_CUDA(cudaEventSynchronize(ctx->ev[0]));
+    ctx->last_iters = h[0].iter;
+    return LQCD_OK;
+}
+
 }  // namespace
 
 // =========================================================================== C-ABI
@@ -394,6 +551,14 @@ int lqcd_create(lqcd_ctx** out, int L0, int L1, int L2, int L3, int fermion_type
     const size_t tables = align_up((size_t)V * 9 * sizeof(int32_t));
     if (tables > stage) stage = tables;
     off += stage;
+    if (fermion_type == LQCD_STAGGERED) {
+        const size_t vecf_bytes = align_up(c->nvec * sizeof(cplxf));
+        c->off_gauge_f = off;  off += align_up((size_t)V * 36 * sizeof(cplxf));
+        c->off_xf = off;       off += vecf_bytes;
+        c->off_rf = off;       off += vecf_bytes;
+        c->off_pf = off;       off += vecf_bytes;
+        c->off_tf = off;       off += vecf_bytes;
+    }
     c->ws_needed = off;
     *out = c;
     return LQCD_OK;
@@ -428,6 +593,7 @@ int lqcd_set_workspace(lqcd_ctx* ctx, void* workspace_dev, size_t bytes, void* c
     ctx->ws = (char*)workspace_dev;
     ctx->stream = (cudaStream_t)cuda_stream;
     ctx->gauge_loaded = false;
+    ctx->gauge_f_ready = false;
     LQCD_CUDA(cudaMemsetAsync(ctx->ws + ctx->off_sc, 0, align_up(sizeof(CgScalars)) + kAlign, ctx->stream));
     return LQCD_OK;
 }
@@ -447,7 +613,7 @@ int lqcd_set_option(lqcd_ctx* ctx, int option, int value)
     }
     if (option == LQCD_OPT_RECONSTRUCT) {
         if (value != 18 && value != 12) return fail(ctx, LQCD_EARG, "reconstruct must be 18 or 12");
-        if (value != ctx->recon) ctx->gauge_loaded = false;  // the internal copy has the other layout
+        if (value != ctx->recon) ctx->gauge_loaded = ctx->gauge_f_ready = false;  // the internal copies have the other layout
         ctx->recon = value;
         return LQCD_OK;
     }
@@ -468,6 +634,7 @@ int lqcd_load_gauge(lqcd_ctx* ctx, const double* u_dev)
         gauge_reorder_kernel<256, kReorderTile, 18, cplx><<<grid, 256, 0, ctx->stream>>>((const cplx*)u_dev, ctx->gauge(),
                                                                                          (size_t)ctx->g.Vh);
     LQCD_LAUNCH_CHECK();
+    ctx->gauge_f_ready = false;
     ctx->gauge_loaded = true;
     return LQCD_OK;
 }
@@ -554,6 +721,41 @@ int lqcd_cg_solve(lqcd_ctx* ctx, double mass_or_kappa, double tol, int maxiter, 
     *iters = h[0].iter;
     *true_residual = h[0].bb > 0.0 ? sqrt(h[0].res2 / h[0].bb) : 0.0;
     const bool converged = h[0].rr_new <= h[0].thresh;
+    return converged ? LQCD_OK : LQCD_MAXITER;
+}
+
+int lqcd_cg_solve_mixed(lqcd_ctx* ctx, double mass, double tol, int maxiter, double delta, const double* b_dev,
+                        double* x_dev, int* iters, int* reliable_updates, double* true_residual)
+{
+    int rc = check_ready(ctx, true);
+    if (rc) return rc;
+    if (ctx->fermion != LQCD_STAGGERED) return fail(ctx, LQCD_EARG, "lqcd_cg_solve_mixed needs a staggered context");
+    if (!b_dev || !x_dev || !iters || !reliable_updates || !true_residual) return fail(ctx, LQCD_EARG, "null pointer argument");
+    if (b_dev == x_dev) return fail(ctx, LQCD_EARG, "b and x must not alias");
+    if (!(tol >= 0.0) || maxiter < 0) return fail(ctx, LQCD_EARG, "tol must be >= 0 and maxiter >= 0");
+    if (!(delta > 0.0 && delta < 1.0)) return fail(ctx, LQCD_EARG, "delta must be in (0,1)");
+    const cplx* b = (const cplx*)b_dev;
+    cplx* x = (cplx*)x_dev;
+    CgScalars* h = ctx->h_sc;
+    rc = cg_run_mixed(ctx, mass, tol, delta, maxiter, b, x);
+    if (rc) return rc;
+    const int it = h[0].iter, nupd = h[0].nupd;
+    const bool converged = h[0].bb == 0.0 || (h[0].rr_new <= h[0].thresh && !h[0].pause && (nupd > 0));
+    // true residual |b - A x| / |b| with a fresh fp64 A (S7)
+    rc = op_first(ctx, mass, x, false);
+    if (rc) return rc;
+    StagArgsD a = stag_args(ctx, LQCD_EVEN, ctx->t(), nullptr);
+    a.m2 = mass * mass;
+    a.p = x;
+    a.b = b;
+    rc = launch_stag<SE_RESIDUAL>(ctx, a);
+    if (rc) return rc;
+    rc = read_scalars(ctx, 0);
+    if (rc) return rc;
+    LQCD_CUDA(cudaEventSynchronize(ctx->ev[0]));
+    *iters = it;
+    *reliable_updates = nupd;
+    *true_residual = h[0].bb > 0.0 ? sqrt(h[0].res2 / h[0].bb) : 0.0;
     return converged ? LQCD_OK : LQCD_MAXITER;
 }
 

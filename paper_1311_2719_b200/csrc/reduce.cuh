@@ -23,12 +23,18 @@ struct CgScalars {
     double beta;      // rr_new / rr
     double thresh;    // tol^2 * bb
     double res2;      // |b - A x|^2 of the final check
-    double aux;       // scratch sum for the stand-alone norm kernel
+    double aux;       // second sum of the two-sum kernels (|b|^2 of the full-system residual)
+    double rmax;      // mixed precision: largest |r| since the last reliable update
+    double delta;     // mixed precision: reliable-update threshold
     int iter;         // completed iterations
     int done;         // 1 once converged (or b = 0): later iterations become no-ops
     int maxiter;
-    int pad;
+    int pause;        // mixed precision: 1 = a reliable update is due; the fp32 iteration kernels are
+                      // no-ops until the update sequence has run (it clears the flag)
+    int nupd;         // mixed precision: reliable updates completed
+    int pad[3];
 };
+static_assert(sizeof(CgScalars) == 128, "CgScalars is copied to the host as one 128-byte block");
 
 struct ReduceScratch {
     double* partials;      // one per block
@@ -49,6 +55,47 @@ __device__ __forceinline__ void cg_after_update(CgScalars* sc, double* hist, dou
     sc->beta = rr_new / sc->rr;
     sc->rr = rr_new;
     if (rr_new <= sc->thresh || it >= sc->maxiter) sc->done = 1;
+}
+
+// Mixed precision: after the fp32 update of xs and rs.  The reliable update
+// is due when the iterated residual has fallen by `delta` below the largest one since the last
+// update, or claims convergence; then the iteration pauses (beta and the p-update wait for the
+// fp64 residual).  Otherwise as cg_after_update, except that convergence is never declared here.
+__device__ __forceinline__ void cg_after_update_mixed(CgScalars* sc, double* hist, double rr_new)
+{
+    const int it = sc->iter + 1;
+    sc->iter = it;
+    sc->rr_new = rr_new;
+    if (it < kHistCap) hist[it] = rr_new;
+    const double rn = sqrt(rr_new);
+    const bool update = rn < sc->delta * sc->rmax || rr_new <= sc->thresh;
+    if (rn > sc->rmax) sc->rmax = rn;
+    if (update) {
+        sc->pause = 1;
+    } else {
+        sc->beta = rr_new / sc->rr;
+        sc->rr = rr_new;
+        if (it >= sc->maxiter) sc->done = 1;
+    }
+}
+
+// After the fp64 residual r = b - A x of a reliable update: |r|^2 replaces the iterated value,
+// convergence is decided on it, and the paused iteration resumes with beta from it.
+__device__ __forceinline__ void cg_after_reliable(CgScalars* sc, double* hist, double rr_true)
+{
+    const int it = sc->iter;
+    sc->rr_new = rr_true;
+    if (it < kHistCap) hist[it] = rr_true;
+    sc->rmax = sqrt(rr_true);
+    sc->nupd += 1;
+    sc->pause = 0;
+    if (rr_true <= sc->thresh) {
+        sc->done = 1;
+    } else {
+        sc->beta = rr_true / sc->rr;
+        sc->rr = rr_true;
+        if (it >= sc->maxiter) sc->done = 1;
+    }
 }
 
 template <int BLOCK>

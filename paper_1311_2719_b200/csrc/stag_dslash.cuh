@@ -27,7 +27,10 @@ enum StagEpilogue {
     // full-system solve M x = b, M = m + D; `m2` carries the mass m here
     SE_PREP = 5,      // out = m p - D in              source preparation  b' = m b_e - D_eo b_o
     SE_RECON = 6,     // out = (p - D in)/m            reconstruction      x_o = (b_o - D_oe x_e)/m
-    SE_RESIDUAL_M = 7 // |b - (m p + D in)|^2 and |b|^2 of one parity, set (flag = 0) or added (flag = 1)
+    SE_RESIDUAL_M = 7, // |b - (m p + D in)|^2 and |b|^2 of one parity, set (flag = 0) or added (flag = 1)
+    // mixed-precision CG with reliable updates
+    SE_CGUPDATE_MIXED = 8,  // SE_CGUPDATE on the fp32 vectors; the scalar step may pause for a reliable update
+    SE_RELIABLE = 9         // fp64: r = b - (m^2 p - D in), rf = fl32(r), |r|^2; resumes the paused iteration
 };
 
 template <class C>
@@ -41,6 +44,7 @@ struct StagArgs {
     C* x;
     C* r;
     const C* b;
+    cplxf* rf;       // SE_RELIABLE: the fp32 residual the inner iteration continues from
     double m2;
     int flag;
     CgScalars* sc;
@@ -101,11 +105,21 @@ __device__ __forceinline__ void stag_hop(const StagArgs<C>& a, const Site& s, C 
 #ifndef LQCD_STAG_MINB12
 #define LQCD_STAG_MINB12 4
 #endif
+#ifndef LQCD_STAG_MINB18F
+#define LQCD_STAG_MINB18F 8
+#endif
+#ifndef LQCD_STAG_MINB12F
+#define LQCD_STAG_MINB12F 8
+#endif
+template <int RECON, class C> struct StagMinBlocks { static constexpr int value = RECON == 12 ? LQCD_STAG_MINB12 : LQCD_STAG_MINB18; };
+template <int RECON> struct StagMinBlocks<RECON, cplxf> { static constexpr int value = RECON == 12 ? LQCD_STAG_MINB12F : LQCD_STAG_MINB18F; };
+
 template <int EPI, int BLOCK, int RECON, class C>
-__global__ void __launch_bounds__(BLOCK, RECON == 12 ? LQCD_STAG_MINB12 : LQCD_STAG_MINB18) stag_dslash_kernel(const StagArgs<C> a)
+__global__ void __launch_bounds__(BLOCK, StagMinBlocks<RECON, C>::value) stag_dslash_kernel(const StagArgs<C> a)
 {
-    if (EPI == SE_NORM || EPI == SE_CGUPDATE) {
-        if (a.sc->done) return;  // converged earlier: this (pre-enqueued) iteration is a no-op
+    if (EPI == SE_NORM || EPI == SE_CGUPDATE || EPI == SE_CGUPDATE_MIXED) {
+        // converged earlier, or waiting for a reliable update: this (pre-enqueued) iteration is a no-op
+        if (a.sc->done | a.sc->pause) return;
     }
     const int e = blockIdx.x * BLOCK + threadIdx.x;
     const bool active = e < a.g.Vh;
@@ -146,7 +160,7 @@ __global__ void __launch_bounds__(BLOCK, RECON == 12 ? LQCD_STAG_MINB12 : LQCD_S
             sc->tt = tt;
             sc->alpha = sc->rr / (m2 * sc->pp + tt);  // <p,Ap> from norms only
         });
-    } else if (EPI == SE_CGUPDATE) {
+    } else if (EPI == SE_CGUPDATE || EPI == SE_CGUPDATE_MIXED) {
         double local = 0.0;
         if (active) {
             const double alpha = a.sc->alpha;
@@ -168,7 +182,25 @@ __global__ void __launch_bounds__(BLOCK, RECON == 12 ? LQCD_STAG_MINB12 : LQCD_S
         }
         CgScalars* sc = a.sc;
         double* hist = a.hist;
-        grid_sum<BLOCK>(local, a.rs, [sc, hist](double rr_new) { cg_after_update(sc, hist, rr_new); });
+        if (EPI == SE_CGUPDATE)
+            grid_sum<BLOCK>(local, a.rs, [sc, hist](double rr_new) { cg_after_update(sc, hist, rr_new); });
+        else
+            grid_sum<BLOCK>(local, a.rs, [sc, hist](double rr_new) { cg_after_update_mixed(sc, hist, rr_new); });
+    } else if (EPI == SE_RELIABLE) {
+        double local = 0.0;
+        if (active) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const size_t i = c * Vh + e;
+                const double2 xv = to_d(a.p[i]), bv = to_d(a.b[i]), q = to_d(acc[c]);
+                const double2 rv = cmake(bv.x - fma(a.m2, xv.x, -q.x), bv.y - fma(a.m2, xv.y, -q.y));
+                a.rf[i] = make_float2((float)rv.x, (float)rv.y);
+                local += cnorm2(rv);
+            }
+        }
+        CgScalars* sc = a.sc;
+        double* hist = a.hist;
+        grid_sum<BLOCK>(local, a.rs, [sc, hist](double rr_true) { cg_after_reliable(sc, hist, rr_true); });
     } else if (EPI == SE_PREP || EPI == SE_RECON) {
         if (active) {
 #pragma unroll

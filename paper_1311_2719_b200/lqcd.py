@@ -68,6 +68,7 @@ def load_library():
     L.lqcd_dslash.argtypes = [P, I, P, P]
     L.lqcd_apply_MdagM.argtypes = [P, D, P, P]
     L.lqcd_cg_solve.argtypes = [P, D, D, I, P, P, ctypes.POINTER(I), ctypes.POINTER(D)]
+    L.lqcd_cg_solve_mixed.argtypes = [P, D, D, I, D, P, P, ctypes.POINTER(I), ctypes.POINTER(I), ctypes.POINTER(D)]
     L.lqcd_stag_solve_full.argtypes = [P, D, D, I, P, P, P, P, ctypes.POINTER(I), ctypes.POINTER(D)]
     L.lqcd_congrad_host.argtypes = [P, P, D, D, I, P, P, ctypes.POINTER(I), ctypes.POINTER(D)]
     L.lqcd_dslash_host.argtypes = [P, I, P, P]
@@ -225,6 +226,22 @@ class Lattice:
                                                  _cptr(x), ctypes.byref(it), ctypes.byref(res)))
         self._sync_out()
         return x, it.value, res.value, rc
+
+    def cg_solve_mixed(self, mass: float, tol: float, maxiter: int, b: torch.Tensor, x: torch.Tensor | None = None,
+                       delta: float = 0.1):
+        """fp32 inner CG with fp64 reliable updates: (x, iters, reliable_updates, true_residual, status)."""
+        self._vec(b, "b")
+        if x is None:
+            x = torch.empty_like(b)
+        self._vec(x, "x")
+        it, nu = ctypes.c_int(0), ctypes.c_int(0)
+        res = ctypes.c_double(0.0)
+        self._sync_in()
+        rc = self._check(self._lib.lqcd_cg_solve_mixed(self._ctx, float(mass), float(tol), int(maxiter), float(delta),
+                                                       _cptr(b), _cptr(x), ctypes.byref(it), ctypes.byref(nu),
+                                                       ctypes.byref(res)))
+        self._sync_out()
+        return x, it.value, nu.value, res.value, rc
 
     def stag_solve_full(self, mass: float, tol: float, maxiter: int, b_even: torch.Tensor, b_odd: torch.Tensor,
                         x_even: torch.Tensor | None = None, x_odd: torch.Tensor | None = None):

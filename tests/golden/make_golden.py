@@ -3,6 +3,8 @@
 the BASELINE.json configs (iteration count, true residual, norm of the solution and a few
 sampled solution entries).  Calls only oracle/ and the seeded input generators; nothing here
 touches the CUDA library.  Usage: python tests/golden/make_golden.py [cfg ...]   (default 1 2 3 4)
+       python tests/golden/make_golden.py --mixed [cfg ...]   adds "cfgN_mixed": the oracle's
+       mixed-precision CG (delta = 0.1) on the staggered configs: iterations, reliable updates, residual.
 
 The full-size GPU tests compare against these instead of re-running minutes of oracle CG.
 LAPACK rounding in the input generators may differ in the last bit between machines; the CG
@@ -25,7 +27,27 @@ OUT = os.path.join(os.path.dirname(os.path.abspath(__file__)), "oracle_cg_refere
 NSAMPLE = 64
 
 
+def mixed(cfgs):
+    ref = json.load(open(OUT)) if os.path.exists(OUT) else {}
+    for n in cfgs:
+        c, u, b = synth.config_inputs(n)
+        assert c["fermion"] == "staggered"
+        t0 = time.time()
+        r = oracle.cg_mixed(c["dims"], u, c["param"], c["tol"], 100000, b, delta=0.1)
+        dt = time.time() - t0
+        x = r["x"].ravel()
+        ref["cfg%d_mixed" % n] = {
+            "delta": 0.1, "iters": r["iters"], "updates": r["updates"], "status": r["status"],
+            "true_residual": r["true_residual"], "x_norm": float(np.linalg.norm(x)), "oracle_seconds": round(dt, 1),
+        }
+        print("cfg%d mixed: iters %d, updates %d, true residual %.3e, %.1f s"
+              % (n, r["iters"], r["updates"], r["true_residual"], dt), flush=True)
+        json.dump(ref, open(OUT, "w"), indent=1, sort_keys=True)
+
+
 def main():
+    if "--mixed" in sys.argv:
+        return mixed([int(a) for a in sys.argv[1:] if a != "--mixed"] or [1, 2, 3])
     cfgs = [int(a) for a in sys.argv[1:]] or [1, 2, 3, 4]
     ref = json.load(open(OUT)) if os.path.exists(OUT) else {}
     for n in cfgs:

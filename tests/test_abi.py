@@ -45,6 +45,8 @@ def test_workspace_size_covers_gauge_vectors_and_staging(dims, fermion):
     v = lat.volume
     nvec = 3 * v // 2 if fermion == 0 else 12 * v
     need = 2 * v * 576 + 5 * nvec * 16          # internal + staged gauge, r p t + staged b x
+    if fermion == 0:
+        need += v * 288 + 4 * nvec * 8           # fp32 links and xs rs ps ts of the mixed-precision solver
     got = lat.workspace_bytes()
     assert need <= got <= need + 4 * 1024 * 1024 + v
     lat.close()
