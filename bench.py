@@ -40,14 +40,20 @@ NOMINAL_HBM_GBS = 8000.0
 FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
 
 
-def cg_bytes(cfg, iters: int, recon: int = 18) -> float:
-    """Algorithmic HBM bytes of one solve; links cost 8 x recon x 8 B per site."""
+def cg_bytes(cfg, iters: int, recon: int = 18, updates: int = -1) -> float:
+    """Algorithmic HBM bytes of one solve; links cost 8 x recon x 8 B per site.
+    updates >= 0: the mixed-precision solver (fp32 iterations + that many fp64 reliable updates)."""
     v = synth.volume(cfg["dims"])
     links = 8 * recon * 8                                 # 1152 B (all nine entries) or 768 B (two rows)
     if cfg["fermion"] == "staggered":
         vh, vec = v // 2, 48
         per_iter = 2 * links + 11 * vec                   # 2832 B / site / iteration at recon 18
         fixed = 4 * vec + (links + 2 * vec) + (links + 4 * vec)  # init + D_oe x + fused residual
+        if updates >= 0:
+            per_iter = per_iter // 2                      # fp32 links and vectors: 1416 / 1032 B
+            # reliable update: x += xs (24 + 2*48), D_oe x (links + 2*48), D_eo + r (links + 3*48 + 24), p-update (3*24)
+            per_update = (24 + 2 * vec) + (links + 2 * vec) + (links + 3 * vec + 24) + 72
+            fixed = (vec + 3 * 24 + vec) + (24 + 2 * vec) + (links + 2 * vec) + (links + 4 * vec) + updates * per_update
         return float(vh) * (per_iter * iters + fixed)
     vec = 192
     per_iter = 2 * links + 11 * vec                       # two full-lattice hops + 11 vector passes
@@ -155,6 +161,10 @@ def main():
     ap.add_argument("--dslash-reps", type=int, default=200)
     ap.add_argument("--recon", type=int, default=18, choices=[18, 12],
                     help="stored reals per link: 18 = all nine entries (the roofline workload), 12 = two rows")
+    ap.add_argument("--precision", default="f64", choices=["f64", "mixed"],
+                    help="f64 = the fp64 conjugate gradient (the headline); mixed = fp32 iterations + fp64 reliable updates")
+    ap.add_argument("--delta", type=float, default=0.1, help="reliable-update threshold of --precision mixed")
+    ap.add_argument("--no-variants", action="store_true", help="skip the extra recon-12 / mixed-precision solves")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -216,10 +226,23 @@ def main():
     v = synth.volume(cfg["dims"])
     sites_out = v // 2   # output sites of one parity Dslash
 
+    mixed = args.precision == "mixed"
+    if mixed and f != lqcd.STAGGERED:
+        raise SystemExit("--precision mixed is built for the staggered configs")
+    updates = -1
+
+    def solve():
+        """One step = one whole solve; returns (iters, reliable updates or -1, true residual, status)."""
+        if mixed:
+            _, it_, nu_, res_, st_ = lat.cg_solve_mixed(cfg["param"], cfg["tol"], maxiter, b_dev, x_dev, delta=args.delta)
+            return it_, nu_, res_, st_
+        _, it_, res_, st_ = lat.cg_solve(cfg["param"], cfg["tol"], maxiter, b_dev, x_dev)
+        return it_, -1, res_, st_
+
     # warm-up
     iters = res = None
     for _ in range(max(args.warmup, 3)):
-        _, iters, res, status = lat.cg_solve(cfg["param"], cfg["tol"], maxiter, b_dev, x_dev)
+        iters, updates, res, status = solve()
     assert status == 0, "CG did not converge"
 
     # ---- timed region 1: K whole solves, device-resident inputs
@@ -229,12 +252,12 @@ def main():
     barrier()
     e0.record(lat.stream)
     for _ in range(args.steps):
-        _, iters, res, status = lat.cg_solve(cfg["param"], cfg["tol"], maxiter, b_dev, x_dev)
+        iters, updates, res, status = solve()
     e1.record(lat.stream)
     barrier()
     ms_solve = max_over_ranks(e0.elapsed_time(e1)) / args.steps
     launches = lat.kernel_launches() - launches0
-    total_bytes = sum_over_ranks(cg_bytes(cfg, iters, args.recon))
+    total_bytes = sum_over_ranks(cg_bytes(cfg, iters, args.recon, updates))
     value = total_bytes / (ms_solve * 1e-3) / 1e9
 
     # ---- timed region 2: the dominant kernel alone (plain Dslash), CUDA events on its stream.
@@ -266,6 +289,7 @@ def main():
     e2e = None
     if not args.no_e2e:
         x_host = torch.empty(lat.vector_shape, dtype=torch.complex128).pin_memory()
+        lat.set_option(lqcd.OPT_CONGRAD_PRECISION, 32 if mixed else 64)
         lat.congrad_host(u_host, cfg["param"], cfg["tol"], maxiter, b_host, x_host)   # warm
         n_e2e = max(1, min(args.steps, 3))
         barrier()
@@ -274,10 +298,39 @@ def main():
             _, it_e, res_e, st_e = lat.congrad_host(u_host, cfg["param"], cfg["tol"], maxiter, b_host, x_host)
         torch.cuda.synchronize()
         sec = max_over_ranks(time.perf_counter() - t0) / n_e2e
-        e2e = {"value": sum_over_ranks(cg_bytes(cfg, it_e, args.recon)) / sec / 1e9, "unit": "GB/s", "ms_per_step": sec * 1e3,
+        e2e = {"value": sum_over_ranks(cg_bytes(cfg, it_e, args.recon, updates)) / sec / 1e9, "unit": "GB/s", "ms_per_step": sec * 1e3,
                "h2d_bytes_per_step": int(u_host.numel() * 16 + b_host.numel() * 16),
-               "d2h_bytes_per_step": int(x_host.numel() * 16 + 96), "iters": it_e, "true_residual": res_e,
+               "d2h_bytes_per_step": int(x_host.numel() * 16 + 128), "iters": it_e, "true_residual": res_e,
                "api": "lqcd_congrad_host (pinned host u, b -> x)"}
+
+    # ---- the other solver variants on the same workload: time-to-solution only (one warm-up, one timed solve)
+    variants = None
+    if f == lqcd.STAGGERED and not args.no_variants:
+        variants = {}
+        for recon_v, prec_v in ((18, "f64"), (12, "f64"), (18, "mixed"), (12, "mixed")):
+            if (recon_v, prec_v) == (args.recon, args.precision):
+                continue
+            lat.set_option(lqcd.OPT_RECONSTRUCT, recon_v)
+            lat.load_gauge(u_dev)
+            v0, v1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            for rep in range(2):
+                barrier()
+                v0.record(lat.stream)
+                if prec_v == "mixed":
+                    _, it_v, nu_v, res_v, st_v = lat.cg_solve_mixed(cfg["param"], cfg["tol"], maxiter, b_dev, x_dev,
+                                                                    delta=args.delta)
+                else:
+                    _, it_v, res_v, st_v = lat.cg_solve(cfg["param"], cfg["tol"], maxiter, b_dev, x_dev)
+                    nu_v = -1
+                v1.record(lat.stream)
+                barrier()
+            ms_v = max_over_ranks(v0.elapsed_time(v1))
+            variants["%s_recon%d" % (prec_v, recon_v)] = {
+                "time_to_solution_ms": ms_v, "iters": it_v, "reliable_updates": nu_v if nu_v >= 0 else None,
+                "true_residual": res_v, "converged": st_v == 0,
+                "GBps": sum_over_ranks(cg_bytes(cfg, it_v, recon_v, nu_v)) / (ms_v * 1e-3) / 1e9}
+        lat.set_option(lqcd.OPT_RECONSTRUCT, args.recon)
+        lat.load_gauge(u_dev)
 
     # ---- the oracle beside it (rank 0, N = 1 only)
     cpu = None
@@ -289,11 +342,13 @@ def main():
         line = {
             "metric": metric, "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_solve, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": workload, "reconstruct": args.recon, "cg_mode": args.cg_mode, "check_every": args.check_every,
+            "vs_baseline": None, "dtype": "f64" if not mixed else "f32 iterations + f64 reliable updates",
+            "data": "synthetic",
+            "config": {"workload": workload, "precision": args.precision, "reconstruct": args.recon, "cg_mode": args.cg_mode, "check_every": args.check_every,
                        "parallelism": "replicas x%d (independent right-hand sides)" % world,
                        "l2_policy": "inputs larger than L2 (%.0f MB of links per Dslash), no flush" % (v * 576 / 1e6)},
-            "cg": {"time_to_solution_ms": ms_solve, "iters": iters, "true_residual": res,
+            "cg": {"time_to_solution_ms": ms_solve, "iters": iters, "reliable_updates": updates if mixed else None,
+                   "true_residual": res,
                    "us_per_iteration": ms_solve * 1e3 / max(iters, 1)},
             "dslash": {"us_per_call": us_dslash, "GBps": achieved, "GFLOPs": dflops * sites_out / (us_dslash * 1e-6) / 1e9,
                        "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS, "reps": args.dslash_reps},
@@ -301,7 +356,7 @@ def main():
                          "wilson_dslash_kernel<WE_PLAIN>", "achieved": achieved, "peak": peak, "unit": "GB/s",
                          "frac": achieved / peak, "peak_source": peak_src, "traffic": None,
                          "bytes_per_site": dbytes, "sites_per_launch": sites_out},
-            "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "cpu_baseline": cpu,
+            "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "cpu_baseline": cpu, "variants": variants,
         }
         line["roofline"]["traffic"] = ncu_traffic("%s_dslash_plain%s" % (cfg["name"], "" if args.recon == 18 else "_recon12"))
         print(json.dumps(line))

@@ -82,7 +82,10 @@ enum {
      * optimisation its code does not use): 96 B per link, 864 instead of
      * 1248 B per staggered Dslash site.  Exact for SU(3) links up to rounding (1e-16).
      * Changing it invalidates the loaded gauge field: call lqcd_load_gauge again. */
-    LQCD_OPT_RECONSTRUCT = 2
+    LQCD_OPT_RECONSTRUCT = 2,
+    /* 64 (default): lqcd_congrad_host solves with lqcd_cg_solve.  32: with lqcd_cg_solve_mixed
+     * (delta = 0.1; staggered contexts only). */
+    LQCD_OPT_CONGRAD_PRECISION = 3
 };
 
 /* Create a context for an L0 x L1 x L2 x L3 lattice (every extent even and >= 2; L = 2 is

@@ -59,6 +59,8 @@ def lib():
         L.oracle_stag_solve_full.argtypes = [P, P, ctypes.c_double, ctypes.c_double, ctypes.c_int, P, P, P, P, P, P]
         L.oracle_stag_dslash_f32.argtypes = [P, P, ctypes.c_int, P, P]
         L.oracle_cg_mixed.argtypes = [P, P, ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_int, P, P, P, P, P, P]
+        L.oracle_wilson_Mhat.argtypes = [P, P, ctypes.c_double, ctypes.c_int, P, P]
+        L.oracle_wilson_solve_eo.argtypes = [P, P, ctypes.c_double, ctypes.c_double, ctypes.c_int, P, P, P, P]
         L.oracle_num_threads.restype = ctypes.c_int
         L.oracle_set_threads.argtypes = [ctypes.c_int]
         _lib = L
@@ -241,3 +243,30 @@ def cg_mixed(dims, u, mass, tol, maxiter, b, delta=0.1, history=False):
     if history:
         out["rr_history"] = hist[: it.value + 1]
     return out
+
+
+def wilson_Mhat(dims, u, kappa, vin, dagger=False):
+    """Schur complement Mhat = 1 - kappa^2 D_eo D_oe (or its adjoint) on the even half of a full-lattice
+    Wilson vector; the odd half of the result is zero."""
+    d = _dims(dims)
+    u = _c(u, np.complex128)
+    vin = _c(vin, np.complex128)
+    assert vin.shape == _vec_shape(dims, WILSON)
+    out = np.empty_like(vin)
+    _check(lib().oracle_wilson_Mhat(_ptr(d), _ptr(u), float(kappa), int(bool(dagger)), _ptr(vin), _ptr(out)),
+           "oracle_wilson_Mhat")
+    return out
+
+
+def wilson_solve_eo(dims, u, kappa, tol, maxiter, b):
+    """M x = b (M = 1 - kappa D_W) by even-odd preconditioning: dict(x, iters, true_residual, status)."""
+    d = _dims(dims)
+    u = _c(u, np.complex128)
+    b = _c(b, np.complex128)
+    assert b.shape == _vec_shape(dims, WILSON)
+    x = np.empty_like(b)
+    it = ctypes.c_int(0)
+    res = ctypes.c_double(0.0)
+    rc = _check(lib().oracle_wilson_solve_eo(_ptr(d), _ptr(u), float(kappa), float(tol), int(maxiter), _ptr(b), _ptr(x),
+                                             ctypes.byref(it), ctypes.byref(res)), "oracle_wilson_solve_eo")
+    return dict(x=x, iters=it.value, true_residual=res.value, status=rc)

@@ -302,25 +302,47 @@ typedef struct {
     int fermion;
     double param; /* mass (staggered) or kappa (Wilson) */
     long n;       /* complex length of a CG vector */
-    cd *t1, *t2;  /* scratch */
+    cd *t1, *t2, *t3; /* scratch */
 } op_t;
+
+/* internal operator type: Schur complement of the Wilson matrix on the even sites (8(f) row 4) */
+#define ORACLE_WILSON_EO 2
 
 static int op_init(op_t *op, const int *L, int fermion, const cd *u, double param)
 {
     if (geom_init(&op->G, L)) return -1;
-    if (fermion != ORACLE_STAGGERED && fermion != ORACLE_WILSON) return -2;
+    if (fermion != ORACLE_STAGGERED && fermion != ORACLE_WILSON && fermion != ORACLE_WILSON_EO) return -2;
     op->u = u;
     op->fermion = fermion;
     op->param = param;
     op->n = fermion == ORACLE_STAGGERED ? 3 * op->G.Vh : 12 * op->G.V;
     op->t1 = malloc(sizeof(cd) * op->n);
     op->t2 = malloc(sizeof(cd) * op->n);
-    return (op->t1 && op->t2) ? 0 : -3;
+    op->t3 = malloc(sizeof(cd) * op->n);
+    return (op->t1 && op->t2 && op->t3) ? 0 : -3;
 }
 static void op_free(op_t *op)
 {
     free(op->t1);
     free(op->t2);
+    free(op->t3);
+}
+
+/* Even-odd (Schur) preconditioned Wilson matrix, SURVEY 8(f) row 4.  In even/odd blocks
+ * M = 1 - kappa D_W = [[1, -kappa D_eo], [-kappa D_oe, 1]], whose Schur complement on the even
+ * sites is  Mhat = 1 - kappa^2 D_eo D_oe.  Vectors are full-lattice arrays of which only the even
+ * half (g < Vh) carries data: out_e = in_e - kappa^2 D_eo D_oe in_e, out_o = 0. */
+static void wilson_Mhat(const geom_t *G, const cd *u, double kappa, const cd *in, cd *out, cd *scratch)
+{
+    wilson_dslash(G, u, 1, in, scratch); /* scratch_o = D_oe in_e */
+    wilson_dslash(G, u, 0, scratch, out); /* out_e = D_eo scratch_o */
+    const long V = G->V, Vh = G->Vh;
+#pragma omp parallel for schedule(static)
+    for (long e = 0; e < Vh; ++e)
+        for (int k = 0; k < 12; ++k) {
+            out[k * V + e] = in[k * V + e] - kappa * kappa * out[k * V + e];
+            out[k * V + Vh + e] = 0;
+        }
 }
 
 /* A = (M^+ M)_ee = m^2 - D_eo D_oe on even-site vectors (staggered);
@@ -334,10 +356,15 @@ static void apply_A(const op_t *op, const cd *in, cd *out)
         stag_dslash(G, op->u, 0, op->t1, op->t2);  /* t2_e = D_eo t1_o */
 #pragma omp parallel for schedule(static)
         for (long i = 0; i < op->n; ++i) out[i] = m2 * in[i] - op->t2[i];
-    } else {
+    } else if (op->fermion == ORACLE_WILSON) {
         wilson_M(G, op->u, op->param, in, op->t1);
         gamma5_mul(G, op->t1, op->t2);
         wilson_M(G, op->u, op->param, op->t2, op->t1);
+        gamma5_mul(G, op->t1, out);
+    } else { /* ORACLE_WILSON_EO: Mhat^+ Mhat = gamma5 Mhat gamma5 Mhat (gamma5 is site-diagonal) */
+        wilson_Mhat(G, op->u, op->param, in, op->t1, op->t3);
+        gamma5_mul(G, op->t1, op->t2);
+        wilson_Mhat(G, op->u, op->param, op->t2, op->t1, op->t3);
         gamma5_mul(G, op->t1, out);
     }
 }
@@ -448,12 +475,10 @@ double oracle_dot_re(const double *a, const double *b, long n_complex)
  * p = r + beta p (missing from the truncated listing; reading A7).
  * Returns 0 = converged, 1 = maxiter reached (outputs valid), <0 = error.
  * rr_hist, if not NULL, receives <r,r> after k iterations at index k (0..iters). */
-int oracle_cg(const int *L, int fermion, const double *u_, double param, double tol, int maxiter, const double *b_,
-              double *x_, int *iters, double *true_res, double *rr_hist)
+static int cg_core(op_t *opp, double tol, int maxiter, const double *b_, double *x_, int *iters, double *true_res,
+                   double *rr_hist)
 {
-    op_t op;
-    int rc = op_init(&op, L, fermion, (const cd *)u_, param);
-    if (rc) return rc;
+#define op (*opp)
     const long n = op.n;
     const cd *b = (const cd *)b_;
     cd *x = (cd *)x_;
@@ -505,8 +530,20 @@ done:
     free(r);
     free(p);
     free(Ap);
-    op_free(&op);
     return status;
+#undef op
+}
+
+int oracle_cg(const int *L, int fermion, const double *u_, double param, double tol, int maxiter, const double *b_,
+              double *x_, int *iters, double *true_res, double *rr_hist)
+{
+    op_t op;
+    if (fermion != ORACLE_STAGGERED && fermion != ORACLE_WILSON) return -2;
+    int rc = op_init(&op, L, fermion, (const cd *)u_, param);
+    if (rc) return rc;
+    rc = cg_core(&op, tol, maxiter, b_, x_, iters, true_res, rr_hist);
+    op_free(&op);
+    return rc;
 }
 
 /* ------------------------------------------------ full-system staggered solve */
@@ -795,6 +832,80 @@ done:
     free(ps);
     free(ts);
     free(qs);
+    op_free(&op);
+    return status;
+}
+
+/* ------------------------------------- even-odd preconditioned Wilson solve */
+
+/* Mhat (dagger = 0) or Mhat^+ = gamma5 Mhat gamma5 (dagger = 1) on the even half of a
+ * full-lattice vector; the odd half of `out` is zero. */
+int oracle_wilson_Mhat(const int *L, const double *u, double kappa, int dagger, const double *in, double *out)
+{
+    op_t op;
+    int rc = op_init(&op, L, ORACLE_WILSON_EO, (const cd *)u, kappa);
+    if (rc) return rc;
+    if (!dagger) {
+        wilson_Mhat(&op.G, op.u, kappa, (const cd *)in, (cd *)out, op.t3);
+    } else {
+        gamma5_mul(&op.G, (const cd *)in, op.t2);
+        wilson_Mhat(&op.G, op.u, kappa, op.t2, op.t1, op.t3);
+        gamma5_mul(&op.G, op.t1, (cd *)out);
+    }
+    op_free(&op);
+    return 0;
+}
+
+/* Solve M x = b, M = 1 - kappa D_W, on the full lattice through the Schur complement on the
+ * even sites.  From  x_e - kappa D_eo x_o = b_e,  x_o - kappa D_oe x_e = b_o:
+ *     x_o = b_o + kappa D_oe x_e,      Mhat x_e = b_e + kappa D_eo b_o,   Mhat = 1 - kappa^2 D_eo D_oe.
+ * Mhat is not hermitian, so the CG runs on its normal equations (as BASELINE.json config 4 does for M).
+ * Steps, in this order:
+ *   1. bh = b_e + kappa D_eo b_o                          (source preparation, even sites)
+ *   2. c  = Mhat^+ bh = gamma5 Mhat gamma5 bh
+ *   3. CG on (Mhat^+ Mhat) x_e = c, 8(c.4) exactly, tol relative to |c|
+ *   4. x_o = b_o + kappa D_oe x_e                         (reconstruction)
+ *   5. true_res = |b - M x| / |b| over the full lattice with M applied afresh
+ * b and x are full-lattice Wilson vectors [4][3][V].  Returns the CG's status. */
+int oracle_wilson_solve_eo(const int *L, const double *u_, double kappa, double tol, int maxiter, const double *b_,
+                           double *x_, int *iters, double *true_res)
+{
+    op_t op;
+    int rc = op_init(&op, L, ORACLE_WILSON_EO, (const cd *)u_, kappa);
+    if (rc) return rc;
+    const geom_t *G = &op.G;
+    const long V = G->V, Vh = G->Vh, n = 12 * V;
+    const cd *u = (const cd *)u_, *b = (const cd *)b_;
+    cd *x = (cd *)x_;
+    cd *bh = malloc(sizeof(cd) * n), *c = malloc(sizeof(cd) * n), *w = malloc(sizeof(cd) * n);
+    if (!bh || !c || !w) return -3;
+    /* 1 */
+    wilson_dslash(G, u, 0, b, w); /* w_e = D_eo b_o */
+    for (int k = 0; k < 12; ++k)
+        for (long e = 0; e < Vh; ++e) {
+            bh[k * V + e] = b[k * V + e] + kappa * w[k * V + e];
+            bh[k * V + Vh + e] = 0;
+        }
+    /* 2 */
+    gamma5_mul(G, bh, w);
+    wilson_Mhat(G, u, kappa, w, c, op.t3);
+    gamma5_mul(G, c, w);
+    memcpy(c, w, sizeof(cd) * n);
+    /* 3: x_e in the even half of x (odd half zero) */
+    double cg_res = 0.0;
+    const int status = cg_core(&op, tol, maxiter, (const double *)c, x_, iters, &cg_res, NULL);
+    /* 4 */
+    wilson_dslash(G, u, 1, x, w); /* w_o = D_oe x_e */
+    for (int k = 0; k < 12; ++k)
+        for (long e = 0; e < Vh; ++e) x[k * V + Vh + e] = b[k * V + Vh + e] + kappa * w[k * V + Vh + e];
+    /* 5 */
+    wilson_M(G, u, kappa, x, w);
+    for (long i = 0; i < n; ++i) w[i] = b[i] - w[i];
+    const double bb = dot_re(b, b, n);
+    *true_res = bb > 0.0 ? sqrt(dot_re(w, w, n) / bb) : 0.0;
+    free(bh);
+    free(c);
+    free(w);
     op_free(&op);
     return status;
 }

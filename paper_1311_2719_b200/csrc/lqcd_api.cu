@@ -51,6 +51,7 @@ struct lqcd_ctx {
     int cg_mode;
     int check_every;
     int recon;  // 18 or 12 stored reals per link
+    int congrad_precision;  // 64 or 32: which solver lqcd_congrad_host runs
     // host side
     CgScalars* h_sc;  // pinned, 2 slots
     cudaEvent_t ev[2];
@@ -532,6 +533,7 @@ int lqcd_create(lqcd_ctx** out, int L0, int L1, int L2, int L3, int fermion_type
     c->cg_mode = LQCD_CG_ASYNC;
     c->check_every = 4;
     c->recon = 18;
+    c->congrad_precision = 64;
 
     size_t off = 0;
     const size_t vec_bytes = align_up(c->nvec * sizeof(cplx));
@@ -615,6 +617,12 @@ int lqcd_set_option(lqcd_ctx* ctx, int option, int value)
         if (value != 18 && value != 12) return fail(ctx, LQCD_EARG, "reconstruct must be 18 or 12");
         if (value != ctx->recon) ctx->gauge_loaded = ctx->gauge_f_ready = false;  // the internal copies have the other layout
         ctx->recon = value;
+        return LQCD_OK;
+    }
+    if (option == LQCD_OPT_CONGRAD_PRECISION) {
+        if (value != 64 && !(value == 32 && ctx->fermion == LQCD_STAGGERED))
+            return fail(ctx, LQCD_EARG, "congrad precision must be 64, or 32 on a staggered context");
+        ctx->congrad_precision = value;
         return LQCD_OK;
     }
     return fail(ctx, LQCD_EARG, "unknown option %d", option);
@@ -833,7 +841,12 @@ int lqcd_congrad_host(lqcd_ctx* ctx, const double* u_host, double mass_or_kappa,
     LQCD_CUDA(cudaMemcpyAsync(sb, b_host, ctx->nvec * sizeof(cplx), cudaMemcpyHostToDevice, ctx->stream));
     rc = lqcd_load_gauge(ctx, (const double*)su);
     if (rc) return rc;
-    const int status = lqcd_cg_solve(ctx, mass_or_kappa, tol, maxiter, (const double*)sb, (double*)sx, iters, true_residual);
+    int nupd = 0;
+    const int status = ctx->congrad_precision == 32
+                           ? lqcd_cg_solve_mixed(ctx, mass_or_kappa, tol, maxiter, 0.1, (const double*)sb, (double*)sx, iters,
+                                                 &nupd, true_residual)
+                           : lqcd_cg_solve(ctx, mass_or_kappa, tol, maxiter, (const double*)sb, (double*)sx, iters,
+                                           true_residual);
     if (status < 0) return status;
     // copyout(x)
     LQCD_CUDA(cudaMemcpyAsync(x_host, sx, ctx->nvec * sizeof(cplx), cudaMemcpyDeviceToHost, ctx->stream));
