@@ -159,6 +159,23 @@ int lqcd_stag_solve_full(lqcd_ctx *ctx, double mass, double tol, int maxiter, co
                          const double *b_odd_dev, double *x_even_dev, double *x_odd_dev, int *iters,
                          double *true_residual);
 
+/* Even-odd (Schur) preconditioned Wilson solver (Wilson contexts).  In even/odd
+ * blocks M = 1 - kappa D_W = [[1, -kappa D_eo], [-kappa D_oe, 1]]; its Schur complement on the even sites is
+ * Mhat = 1 - kappa^2 D_eo D_oe, with Mhat^+ = gamma5 Mhat gamma5.  Vectors are full-lattice Wilson
+ * vectors [4][3][V]; "even half" = the entries with site index g < Vh.
+ *
+ * lqcd_wilson_eo_MdagM: even half of out = Mhat^+ Mhat applied to the even half of in; the odd halves
+ * are neither read nor written.  No aliasing.
+ *
+ * lqcd_wilson_solve_eo: solves M x = b on the full lattice:  bh = b_e + kappa D_eo b_o;  c = Mhat^+ bh;
+ * CG (as lqcd_cg_solve, tol relative to |c|) on Mhat^+ Mhat x_e = c;  x_o = b_o + kappa D_oe x_e;
+ * *true_residual = |b - M x| / |b| over the full lattice with M applied afresh.  *iters = CG iterations
+ * (each costs the same four one-parity hopping terms as an iteration of lqcd_cg_solve, on a better
+ * conditioned matrix).  b = 0 gives x = 0. */
+int lqcd_wilson_eo_MdagM(lqcd_ctx *ctx, double kappa, const double *in_dev, double *out_dev);
+int lqcd_wilson_solve_eo(lqcd_ctx *ctx, double kappa, double tol, int maxiter, const double *b_dev, double *x_dev,
+                         int *iters, double *true_residual);
+
 /* The paper's congrad with its data region (copyin(u,r) ... copyout(x)):
  * HOST buffers in the canonical layouts (pinned memory makes the copies asynchronous).
  * Copies u and b to the device, converts the gauge field, solves, copies x back. */

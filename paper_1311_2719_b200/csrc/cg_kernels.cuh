@@ -5,16 +5,30 @@
 
 namespace lqcd {
 
+// Which elements of the arrays make up a CG vector: n elements in runs of `inner`, the runs `stride`
+// apart.  Contiguous vectors: inner = stride = n.  The even half of a full-lattice Wilson vector
+// [12][V] (even-odd preconditioned solver): n = 12 Vh, inner = Vh, stride = V.
+struct VecLayout {
+    size_t n, inner, stride;
+    __device__ __forceinline__ size_t at(size_t j) const
+    {
+        if (inner == n) return j;
+        const size_t k = j / inner;
+        return k * stride + (j - k * inner);
+    }
+};
+
 // S6: p = r = b, x = 0, betan = <r,r> in one pass; also bb, pp and the CG
-// bookkeeping.  n = number of complex elements of a CG vector.
+// bookkeeping.
 template <int BLOCK>
 __global__ void __launch_bounds__(BLOCK) cg_init_kernel(const cplx* __restrict__ b, cplx* __restrict__ x,
-                                                        cplx* __restrict__ r, cplx* __restrict__ p, size_t n,
+                                                        cplx* __restrict__ r, cplx* __restrict__ p, VecLayout lay,
                                                         CgScalars* sc, ReduceScratch rs, double* hist, double tol,
                                                         int maxiter)
 {
     double local = 0.0;
-    for (size_t i = (size_t)blockIdx.x * BLOCK + threadIdx.x; i < n; i += (size_t)gridDim.x * BLOCK) {
+    for (size_t j = (size_t)blockIdx.x * BLOCK + threadIdx.x; j < lay.n; j += (size_t)gridDim.x * BLOCK) {
+        const size_t i = lay.at(j);
         const cplx v = b[i];
         r[i] = v;
         p[i] = v;
@@ -113,13 +127,14 @@ __global__ void gauge_narrow_kernel(const cplx* __restrict__ g64, cplxf* __restr
 // C = cplx (the fp64 path) or cplxf (the fp32 inner iteration: evaluated in fp64, rounded on store,
 // the norm taken of the stored value).
 template <int BLOCK, class C>
-__global__ void __launch_bounds__(BLOCK) cg_pupdate_kernel(const C* __restrict__ r, C* __restrict__ p, size_t n,
+__global__ void __launch_bounds__(BLOCK) cg_pupdate_kernel(const C* __restrict__ r, C* __restrict__ p, VecLayout lay,
                                                            CgScalars* sc, ReduceScratch rs)
 {
     if (sc->done | sc->pause) return;
     const double beta = sc->beta;
     double local = 0.0;
-    for (size_t i = (size_t)blockIdx.x * BLOCK + threadIdx.x; i < n; i += (size_t)gridDim.x * BLOCK) {
+    for (size_t j = (size_t)blockIdx.x * BLOCK + threadIdx.x; j < lay.n; j += (size_t)gridDim.x * BLOCK) {
+        const size_t i = lay.at(j);
         const double2 rv = to_d(r[i]);
         double2 pv = to_d(p[i]);
         pv.x = fma(beta, pv.x, rv.x);

@@ -52,6 +52,7 @@ struct lqcd_ctx {
     int check_every;
     int recon;  // 18 or 12 stored reals per link
     int congrad_precision;  // 64 or 32: which solver lqcd_congrad_host runs
+    bool wilson_eo;  // set while lqcd_wilson_solve_eo runs: the CG works on Mhat^+ Mhat, even half of the vectors
     // host side
     CgScalars* h_sc;  // pinned, 2 slots
     cudaEvent_t ev[2];
@@ -120,9 +121,22 @@ int check_ready(lqcd_ctx* ctx, bool need_gauge)
 
 unsigned int blocks_for(size_t n, int block) { return (unsigned int)((n + block - 1) / block); }
 
+VecLayout vec_layout(const lqcd_ctx* ctx)
+{
+    VecLayout l;
+    if (ctx->wilson_eo) {
+        l.n = 12 * (size_t)ctx->g.Vh;
+        l.inner = (size_t)ctx->g.Vh;
+        l.stride = (size_t)ctx->g.V;
+    } else {
+        l.n = l.inner = l.stride = ctx->nvec;
+    }
+    return l;
+}
+
 unsigned int vec_grid(const lqcd_ctx* ctx)
 {
-    size_t b = (ctx->nvec + kVecBlock - 1) / kVecBlock;
+    size_t b = (vec_layout(ctx).n + kVecBlock - 1) / kVecBlock;
     const size_t cap = 148 * 8;
     if (b > cap) b = cap;
     if (b < 1) b = 1;
@@ -205,7 +219,7 @@ WilsonArgs wilson_args(const lqcd_ctx* ctx, int parity, const cplx* in, cplx* ou
 template <int EPI, bool DAGGER>
 int launch_wilson(lqcd_ctx* ctx, const WilsonArgs& a)
 {
-    const size_t n = EPI == WE_PLAIN ? (size_t)ctx->g.Vh : (size_t)ctx->g.V;
+    const size_t n = wilson_one_parity(EPI) ? (size_t)ctx->g.Vh : (size_t)ctx->g.V;
     const unsigned int grid = blocks_for(n, kWilsonBlock);
     if (ctx->recon == 12)
         wilson_dslash_kernel<EPI, DAGGER, kWilsonBlock, 12><<<grid, kWilsonBlock, 0, ctx->stream>>>(a);
@@ -228,8 +242,37 @@ int op_first(lqcd_ctx* ctx, double param, const cplx* v, bool with_norm)
     return with_norm ? launch_wilson<WE_M_NORM, false>(ctx, a) : launch_wilson<WE_M, false>(ctx, a);
 }
 
+// Even-odd preconditioned Wilson: t_e = Mhat v_e (DAGGER = false) or Mhat^+ v_e
+// (true), Mhat = 1 - kappa^2 D_eo D_oe, through the odd half of the scratch vector t.  `dst` receives
+// the even half of the result; with_norm adds tt = |result|^2 and alpha = rr/tt.
+template <bool DAGGER>
+int eo_mhat(lqcd_ctx* ctx, double kappa, const cplx* v, cplx* dst, bool with_norm)
+{
+    int rc = launch_wilson<WE_PLAIN, DAGGER>(ctx, wilson_args(ctx, LQCD_ODD, v, ctx->t(), 0.0));
+    if (rc) return rc;
+    WilsonArgs a = wilson_args(ctx, LQCD_EVEN, ctx->t(), dst, -kappa * kappa);
+    a.p = v;
+    return with_norm ? launch_wilson<WE_EO_XPAY_NORM, DAGGER>(ctx, a) : launch_wilson<WE_EO_XPAY, DAGGER>(ctx, a);
+}
+
+int eo_iteration_kernels(lqcd_ctx* ctx, double kappa, cplx* x)
+{
+    int rc = eo_mhat<false>(ctx, kappa, ctx->p(), ctx->t(), true);  // t_e = Mhat p, alpha = rr/|t_e|^2
+    if (rc) return rc;
+    // w_o = D^+_oe t_e into the odd half of t; Ap = t_e - kappa^2 D^+_eo w_o fused with the x / r updates
+    rc = launch_wilson<WE_PLAIN, true>(ctx, wilson_args(ctx, LQCD_ODD, ctx->t(), ctx->t(), 0.0));
+    if (rc) return rc;
+    WilsonArgs a = wilson_args(ctx, LQCD_EVEN, ctx->t(), nullptr, -kappa * kappa);
+    a.p = ctx->t();
+    a.b = ctx->p();
+    a.x = x;
+    a.r = ctx->r();
+    return launch_wilson<WE_EO_CGUPDATE, true>(ctx, a);
+}
+
 int cg_iteration_kernels(lqcd_ctx* ctx, double param, cplx* x)
 {
+    if (ctx->wilson_eo) return eo_iteration_kernels(ctx, param, x);
     int rc = op_first(ctx, param, ctx->p(), true);  // S1 + S2
     if (rc) return rc;
     if (ctx->fermion == LQCD_STAGGERED) {           // S3
@@ -249,7 +292,7 @@ int cg_iteration_kernels(lqcd_ctx* ctx, double param, cplx* x)
 
 int cg_pupdate(lqcd_ctx* ctx)  // S5
 {
-    cg_pupdate_kernel<kVecBlock, cplx><<<vec_grid(ctx), kVecBlock, 0, ctx->stream>>>(ctx->r(), ctx->p(), ctx->nvec, ctx->sc(),
+    cg_pupdate_kernel<kVecBlock, cplx><<<vec_grid(ctx), kVecBlock, 0, ctx->stream>>>(ctx->r(), ctx->p(), vec_layout(ctx), ctx->sc(),
                                                                               ctx->rs());
     LQCD_LAUNCH_CHECK();
     return LQCD_OK;
@@ -299,7 +342,7 @@ int cg_run(lqcd_ctx* ctx, double mass_or_kappa, double tol, int maxiter, const c
 {
     int rc;
     // S6: p = r = b, x = 0, rr = bb = pp = |b|^2
-    cg_init_kernel<kVecBlock><<<vec_grid(ctx), kVecBlock, 0, ctx->stream>>>(b, x, ctx->r(), ctx->p(), ctx->nvec, ctx->sc(),
+    cg_init_kernel<kVecBlock><<<vec_grid(ctx), kVecBlock, 0, ctx->stream>>>(b, x, ctx->r(), ctx->p(), vec_layout(ctx), ctx->sc(),
                                                                            ctx->rs(), ctx->hist(), tol, maxiter);
     LQCD_LAUNCH_CHECK();
 
@@ -348,7 +391,7 @@ int cg_run(lqcd_ctx* ctx, double mass_or_kappa, double tol, int maxiter, const c
             if (enqueued < (long long)maxiter) {
                 if (gh.exec) {
                     LQCD_CUDA(cudaGraphLaunch(gh.exec, ctx->stream));
-                    ctx->launches += 3LL * batch;
+                    ctx->launches += (ctx->wilson_eo ? 5LL : 3LL) * batch;
                 } else {
                     rc = enqueue_batch(ctx, mass_or_kappa, x, batch);
                     if (rc) return rc;
@@ -394,7 +437,7 @@ int mixed_iteration_kernels(lqcd_ctx* ctx, double mass)  // S1 + S2, S3 on the f
 
 int mixed_pupdate(lqcd_ctx* ctx)  // S5 on the fp32 copies
 {
-    cg_pupdate_kernel<kVecBlock, cplxf><<<vec_grid(ctx), kVecBlock, 0, ctx->stream>>>(ctx->rf(), ctx->pf(), ctx->nvec,
+    cg_pupdate_kernel<kVecBlock, cplxf><<<vec_grid(ctx), kVecBlock, 0, ctx->stream>>>(ctx->rf(), ctx->pf(), vec_layout(ctx),
                                                                                       ctx->sc(), ctx->rs());
     LQCD_LAUNCH_CHECK();
     return LQCD_OK;
@@ -818,6 +861,75 @@ int lqcd_stag_solve_full(lqcd_ctx* ctx, double mass, double tol, int maxiter, co
     a.flag = 1;
     rc = launch_stag<SE_RESIDUAL_M>(ctx, a);
     if (rc) return rc;
+    rc = read_scalars(ctx, 0);
+    if (rc) return rc;
+    LQCD_CUDA(cudaEventSynchronize(ctx->ev[0]));
+    *iters = cg_iters;
+    *true_residual = h[0].aux > 0.0 ? sqrt(h[0].res2 / h[0].aux) : 0.0;
+    return converged ? LQCD_OK : LQCD_MAXITER;
+}
+
+int lqcd_wilson_eo_MdagM(lqcd_ctx* ctx, double kappa, const double* in_dev, double* out_dev)
+{
+    int rc = check_ready(ctx, true);
+    if (rc) return rc;
+    if (ctx->fermion != LQCD_WILSON) return fail(ctx, LQCD_EARG, "lqcd_wilson_eo_MdagM needs a Wilson context");
+    if (!in_dev || !out_dev) return fail(ctx, LQCD_EARG, "null vector pointer");
+    if (in_dev == out_dev) return fail(ctx, LQCD_EARG, "in and out must not alias");
+    rc = eo_mhat<false>(ctx, kappa, (const cplx*)in_dev, ctx->t(), false);  // t_e = Mhat in_e
+    if (rc) return rc;
+    // out_e = Mhat^+ t_e: w_o = D^+_oe t_e into the odd half of t, then the diagonal term from t_e
+    rc = launch_wilson<WE_PLAIN, true>(ctx, wilson_args(ctx, LQCD_ODD, ctx->t(), ctx->t(), 0.0));
+    if (rc) return rc;
+    WilsonArgs a = wilson_args(ctx, LQCD_EVEN, ctx->t(), (cplx*)out_dev, -kappa * kappa);
+    a.p = ctx->t();
+    return launch_wilson<WE_EO_XPAY, true>(ctx, a);
+}
+
+int lqcd_wilson_solve_eo(lqcd_ctx* ctx, double kappa, double tol, int maxiter, const double* b_dev, double* x_dev,
+                         int* iters, double* true_residual)
+{
+    int rc = check_ready(ctx, true);
+    if (rc) return rc;
+    if (ctx->fermion != LQCD_WILSON) return fail(ctx, LQCD_EARG, "lqcd_wilson_solve_eo needs a Wilson context");
+    if (!b_dev || !x_dev || !iters || !true_residual) return fail(ctx, LQCD_EARG, "null pointer argument");
+    if (b_dev == x_dev) return fail(ctx, LQCD_EARG, "b and x must not alias");
+    if (!(tol >= 0.0) || maxiter < 0) return fail(ctx, LQCD_EARG, "tol must be >= 0 and maxiter >= 0");
+    const cplx* b = (const cplx*)b_dev;
+    cplx* x = (cplx*)x_dev;
+    cplx* bh = (cplx*)(ctx->ws + ctx->off_stage_b);  // staging vectors are idle during device-pointer calls
+    cplx* c = (cplx*)(ctx->ws + ctx->off_stage_x);
+    CgScalars* h = ctx->h_sc;
+
+    // 1. bh_e = b_e + kappa D_eo b_o
+    WilsonArgs a = wilson_args(ctx, LQCD_EVEN, b, bh, kappa);
+    a.p = b;
+    rc = launch_wilson<WE_EO_XPAY, false>(ctx, a);
+    if (rc) return rc;
+    // 2. c_e = Mhat^+ bh_e
+    rc = eo_mhat<true>(ctx, kappa, bh, c, false);
+    if (rc) return rc;
+    // 3. CG on Mhat^+ Mhat x_e = c_e over the even half of the full-lattice arrays
+    ctx->wilson_eo = true;
+    rc = cg_run(ctx, kappa, tol, maxiter, c, x);
+    ctx->wilson_eo = false;
+    if (rc) return rc;
+    const int cg_iters = h[0].iter;
+    const bool converged = h[0].rr_new <= h[0].thresh;
+    // 4. x_o = b_o + kappa D_oe x_e
+    a = wilson_args(ctx, LQCD_ODD, x, x, kappa);
+    a.p = b;
+    rc = launch_wilson<WE_EO_XPAY, false>(ctx, a);
+    if (rc) return rc;
+    // 5. |b - M x|^2 and |b|^2, M = 1 - kappa D_W, one parity at a time
+    for (int parity = 0; parity < 2; ++parity) {
+        a = wilson_args(ctx, parity, x, nullptr, -kappa);
+        a.p = x;
+        a.b = b;
+        a.flag = parity;
+        rc = launch_wilson<WE_EO_RESIDUAL, false>(ctx, a);
+        if (rc) return rc;
+    }
     rc = read_scalars(ctx, 0);
     if (rc) return rc;
     LQCD_CUDA(cudaEventSynchronize(ctx->ev[0]));

@@ -22,8 +22,17 @@ enum WilsonEpilogue {
     WE_M = 1,         // out = in - kappa D in, full lattice
     WE_M_NORM = 2,    // the same + tt = |out|^2, alpha = rr/tt                 (S1, S2: <p,Ap> = |Mp|^2)
     WE_CGUPDATE = 3,  // Ap = in - kappa D^+ in; x += alpha p; r -= alpha Ap; |r|^2   (S3)
-    WE_RESIDUAL = 4   // |b - (in - kappa D^+ in)|^2                            (S7)
+    WE_RESIDUAL = 4,  // |b - (in - kappa D^+ in)|^2                            (S7)
+    // One-parity kernels of the even-odd (Schur) preconditioned solver, SURVEY.md 8(f) row 4.  `p` is the
+    // site-diagonal operand on the output parity, `kappa` carries the coefficient c of  d = p + c * (D in):
+    // c = -kappa^2 for Mhat = 1 - kappa^2 D_eo D_oe, c = +kappa for the source preparation and the
+    // reconstruction, c = -kappa for the rows of M itself.
+    WE_EO_XPAY = 5,       // out = d
+    WE_EO_XPAY_NORM = 6,  // out = d, tt = |d|^2, alpha = rr/tt                 (<p, Mhat^+ Mhat p> = |Mhat p|^2)
+    WE_EO_CGUPDATE = 7,   // Ap = d; x += alpha q; r -= alpha Ap; |r|^2         (q = the search direction, in `b`)
+    WE_EO_RESIDUAL = 8    // |b - d|^2 and |b|^2 of one parity, set (flag = 0) or added (flag = 1)
 };
+__host__ __device__ constexpr bool wilson_one_parity(int epi) { return epi == WE_PLAIN || epi >= WE_EO_XPAY; }
 
 struct WilsonArgs {
     Geom g;
@@ -36,6 +45,7 @@ struct WilsonArgs {
     cplx* r;
     const cplx* b;
     double kappa;
+    int flag;
     CgScalars* sc;
     ReduceScratch rs;
     double* hist;
@@ -112,14 +122,14 @@ __device__ __forceinline__ void wilson_dir(const WilsonArgs& a, const Site& s, i
 template <int EPI, bool DAGGER, int BLOCK, int RECON>
 __global__ void __launch_bounds__(BLOCK) wilson_dslash_kernel(const WilsonArgs a)
 {
-    if (EPI == WE_M_NORM || EPI == WE_CGUPDATE) {
+    if (EPI == WE_M_NORM || EPI == WE_CGUPDATE || EPI == WE_EO_XPAY_NORM || EPI == WE_EO_CGUPDATE) {
         if (a.sc->done) return;
     }
     const long long idx = (long long)blockIdx.x * BLOCK + threadIdx.x;
     const size_t Vh = (size_t)a.g.Vh, V = (size_t)a.g.V;
     bool active;
     int parity, e;
-    if (EPI == WE_PLAIN) {
+    if (wilson_one_parity(EPI)) {
         active = idx < (long long)Vh;
         parity = a.parity;
         e = (int)idx;
@@ -147,6 +157,55 @@ __global__ void __launch_bounds__(BLOCK) wilson_dslash_kernel(const WilsonArgs a
         if (active) {
 #pragma unroll
             for (int k = 0; k < 12; ++k) st_vec(a.out + (size_t)k * V + gsite, acc[k / 3][k % 3]);
+        }
+        return;
+    }
+    if (EPI >= WE_EO_XPAY) {
+        // one-parity forms: d = p + c * acc
+        double local[2] = { 0.0, 0.0 };
+        const double alpha = (EPI == WE_EO_CGUPDATE && active) ? a.sc->alpha : 0.0;
+        if (active) {
+#pragma unroll
+            for (int k = 0; k < 12; ++k) {
+                const size_t i = (size_t)k * V + gsite;
+                const cplx c0 = a.p[i];
+                const cplx d = cmake(fma(a.kappa, acc[k / 3][k % 3].x, c0.x), fma(a.kappa, acc[k / 3][k % 3].y, c0.y));
+                if (EPI == WE_EO_XPAY || EPI == WE_EO_XPAY_NORM) {
+                    st_vec(a.out + i, d);
+                    if (EPI == WE_EO_XPAY_NORM) local[0] += cnorm2(d);
+                } else if (EPI == WE_EO_CGUPDATE) {
+                    const cplx qv = a.b[i];
+                    cplx xv = a.x[i], rv = a.r[i];
+                    xv.x = fma(alpha, qv.x, xv.x);
+                    xv.y = fma(alpha, qv.y, xv.y);
+                    rv.x = fma(-alpha, d.x, rv.x);
+                    rv.y = fma(-alpha, d.y, rv.y);
+                    a.x[i] = xv;
+                    a.r[i] = rv;
+                    local[0] += cnorm2(rv);
+                } else {  // WE_EO_RESIDUAL
+                    const cplx bv = a.b[i];
+                    const double re = bv.x - d.x, im = bv.y - d.y;
+                    local[0] += fma(re, re, im * im);
+                    local[1] += cnorm2(bv);
+                }
+            }
+        }
+        CgScalars* sc = a.sc;
+        if (EPI == WE_EO_XPAY_NORM) {
+            grid_sum<BLOCK>(local[0], a.rs, [sc](double tt) {
+                sc->tt = tt;
+                sc->alpha = sc->rr / tt;
+            });
+        } else if (EPI == WE_EO_CGUPDATE) {
+            double* hist = a.hist;
+            grid_sum<BLOCK>(local[0], a.rs, [sc, hist](double rr_new) { cg_after_update(sc, hist, rr_new); });
+        } else if (EPI == WE_EO_RESIDUAL) {
+            const int add = a.flag;
+            grid_sum_n<BLOCK, 2>(local, a.rs, [sc, add](const double (&tot)[2]) {
+                sc->res2 = add ? sc->res2 + tot[0] : tot[0];
+                sc->aux = add ? sc->aux + tot[1] : tot[1];
+            });
         }
         return;
     }

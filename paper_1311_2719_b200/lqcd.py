@@ -70,6 +70,8 @@ def load_library():
     L.lqcd_cg_solve.argtypes = [P, D, D, I, P, P, ctypes.POINTER(I), ctypes.POINTER(D)]
     L.lqcd_cg_solve_mixed.argtypes = [P, D, D, I, D, P, P, ctypes.POINTER(I), ctypes.POINTER(I), ctypes.POINTER(D)]
     L.lqcd_stag_solve_full.argtypes = [P, D, D, I, P, P, P, P, ctypes.POINTER(I), ctypes.POINTER(D)]
+    L.lqcd_wilson_eo_MdagM.argtypes = [P, D, P, P]
+    L.lqcd_wilson_solve_eo.argtypes = [P, D, D, I, P, P, ctypes.POINTER(I), ctypes.POINTER(D)]
     L.lqcd_congrad_host.argtypes = [P, P, D, D, I, P, P, ctypes.POINTER(I), ctypes.POINTER(D)]
     L.lqcd_dslash_host.argtypes = [P, I, P, P]
     L.lqcd_cg_history.argtypes = [P, P, I]
@@ -258,6 +260,31 @@ class Lattice:
                                                         ctypes.byref(res)))
         self._sync_out()
         return x_even, x_odd, it.value, res.value, rc
+
+    def wilson_eo_MdagM(self, kappa: float, vin: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:
+        """Even half of out = Mhat^+ Mhat (even half of vin); a fresh `out` has a zero odd half."""
+        self._vec(vin, "in")
+        if out is None:
+            out = torch.zeros_like(vin)
+        self._vec(out, "out")
+        self._sync_in()
+        self._check(self._lib.lqcd_wilson_eo_MdagM(self._ctx, float(kappa), _cptr(vin), _cptr(out)))
+        self._sync_out()
+        return out
+
+    def wilson_solve_eo(self, kappa: float, tol: float, maxiter: int, b: torch.Tensor, x: torch.Tensor | None = None):
+        """M x = b (M = 1 - kappa D_W) by even-odd preconditioning: (x, iters, true_residual, status)."""
+        self._vec(b, "b")
+        if x is None:
+            x = torch.empty_like(b)
+        self._vec(x, "x")
+        it = ctypes.c_int(0)
+        res = ctypes.c_double(0.0)
+        self._sync_in()
+        rc = self._check(self._lib.lqcd_wilson_solve_eo(self._ctx, float(kappa), float(tol), int(maxiter), _cptr(b),
+                                                        _cptr(x), ctypes.byref(it), ctypes.byref(res)))
+        self._sync_out()
+        return x, it.value, res.value, rc
 
     def congrad_host(self, u_host: torch.Tensor, mass_or_kappa: float, tol: float, maxiter: int, b_host: torch.Tensor,
                      x_host: torch.Tensor | None = None):
