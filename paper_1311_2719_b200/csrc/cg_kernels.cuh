@@ -114,7 +114,7 @@ __global__ void __launch_bounds__(BLOCK) mixed_accumulate_kernel(cplx* __restric
 }
 
 // fp64 structure-of-arrays links -> fp32 copy of the same layout (built once per loaded gauge field).
-__global__ void gauge_narrow_kernel(const cplx* __restrict__ g64, cplxf* __restrict__ g32, size_t n)
+static __global__ void gauge_narrow_kernel(const cplx* __restrict__ g64, cplxf* __restrict__ g32, size_t n)
 {
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
         const cplx v = g64[i];
@@ -174,7 +174,7 @@ __global__ void __launch_bounds__(BLOCK) gauge_reorder_kernel(const cplx* __rest
 
 // The paper's iup / idn as g-indices, from the same nbr_fwd / nbr_bwd the
 // Dslash kernels use, plus lex2eo[s] = g.
-__global__ void tables_kernel(Geom g, int32_t* __restrict__ iup, int32_t* __restrict__ idn,
+static __global__ void tables_kernel(Geom g, int32_t* __restrict__ iup, int32_t* __restrict__ idn,
                               int32_t* __restrict__ lex2eo)
 {
     const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;

@@ -1,0 +1,779 @@
+// lqcd_slab.cu -- the C-ABI of include/lqcd_slab.h: the staggered conjugate gradient of the paper
+// on a lattice cut into time-slabs, one per GPU.
+// Every entry point is a thin wrapper around a *_group function that drives n slabs phase by phase;
+// the one-rank-per-process calls are the n = 1 case of the same code.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include "../../include/lqcd_slab.h"
+#include "slab_kernels.cuh"
+#include "stag_dslash.cuh"
+
+using namespace lqcd;
+
+namespace {
+constexpr int kStagBlock = 128;
+constexpr int kVecBlock = 256;
+constexpr int kReorderTile = 64;
+constexpr size_t kAlign = 256;
+typedef StagArgs<cplx> StagArgsD;
+size_t align_up(size_t n) { return (n + kAlign - 1) / kAlign * kAlign; }
+unsigned int blocks_for(size_t n, int block) { return (unsigned int)((n + block - 1) / block); }
+}  // namespace
+
+struct lqcd_slab {
+    int L[4];
+    int rank, nranks, T, t0, sh;
+    Geom g;       // the LOCAL lattice L0 x L1 x L2 x T
+    size_t nvec;  // complex numbers per local vector
+    // workspace (private) byte offsets
+    size_t off_gauge, off_gghost, off_r, off_p, off_t, off_sc, off_ss, off_ticket, off_partials, off_hist, ws_needed;
+    // mailbox (peer-visible) byte offsets
+    size_t mb_flag, mb_slot, mb_ghost, mb_needed;
+    size_t max_blocks;
+    char* ws;
+    char* mb;
+    char* peer[LQCD_SLAB_MAX_RANKS];
+    cudaStream_t stream;
+    int device;
+    bool memory_set, connected, gauge_loaded;
+    int recon, check_every, timeout_ms;
+    unsigned long long seq;  // synchronisation points passed
+    CgScalars* h_sc;         // pinned, 2 slots
+    SlabScalars* h_ss;       // pinned
+    cudaEvent_t ev[2];
+    bool host_ready;
+    long long launches;
+    char err[320];
+
+    cplx* gauge() const { return (cplx*)(ws + off_gauge); }
+    cplx* gghost() const { return (cplx*)(ws + off_gghost); }
+    cplx* r() const { return (cplx*)(ws + off_r); }
+    cplx* p() const { return (cplx*)(ws + off_p); }
+    cplx* t() const { return (cplx*)(ws + off_t); }
+    CgScalars* sc() const { return (CgScalars*)(ws + off_sc); }
+    SlabScalars* ss() const { return (SlabScalars*)(ws + off_ss); }
+    double* hist() const { return (double*)(ws + off_hist); }
+    ReduceScratch rs() const
+    {
+        ReduceScratch q;
+        q.partials = (double*)(ws + off_partials);
+        q.ticket = (unsigned int*)(ws + off_ticket);
+        return q;
+    }
+    // ghost face `side` (0 = below the slab, 1 = above) of buffer `buf` in the mailbox at `base`
+    cplx* ghost(char* base, int buf, int side) const
+    {
+        return (cplx*)(base + mb_ghost) + (size_t)(buf * 2 + side) * 3 * (size_t)sh;
+    }
+};
+
+namespace {
+
+int fail(lqcd_slab* s, int code, const char* fmt, ...)
+{
+    if (s) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(s->err, sizeof s->err, fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+#define SLAB_CUDA(call)                                                                                \
+    do {                                                                                               \
+        cudaError_t e_ = (call);                                                                       \
+        if (e_ != cudaSuccess)                                                                         \
+            return fail(s, LQCD_ECUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, \
+                        __LINE__);                                                                     \
+    } while (0)
+
+#define SLAB_LAUNCH_CHECK()                                                                            \
+    do {                                                                                               \
+        s->launches++;                                                                                 \
+        cudaError_t e_ = cudaGetLastError();                                                           \
+        if (e_ != cudaSuccess)                                                                         \
+            return fail(s, LQCD_ECUDA, "kernel launch failed: %s (%s:%d)", cudaGetErrorString(e_),     \
+                        __FILE__, __LINE__);                                                           \
+    } while (0)
+
+unsigned int vec_grid(const lqcd_slab* s)
+{
+    size_t b = (s->nvec + kVecBlock - 1) / kVecBlock;
+    const size_t cap = 148 * 8;
+    if (b > cap) b = cap;
+    if (b < 1) b = 1;
+    return (unsigned int)b;
+}
+
+// The n slabs of a *_group call.
+struct Group {
+    lqcd_slab* const* s;
+    int n;
+};
+
+int group_check(const Group& G, bool need_gauge)
+{
+    if (!G.s || G.n < 1) return LQCD_EARG;
+    for (int r = 0; r < G.n; ++r)
+        if (!G.s[r]) return LQCD_EARG;
+    for (int r = 0; r < G.n; ++r) {
+        lqcd_slab* s = G.s[r];
+        if (s->nranks != G.n || s->rank != r)
+            return fail(s, LQCD_EARG, "group of %d slabs: entry %d is rank %d of %d", G.n, r, s->rank, s->nranks);
+        if (!s->memory_set) return fail(s, LQCD_ESTATE, "memory not set (call lqcd_slab_set_memory)");
+        if (!s->connected) return fail(s, LQCD_ESTATE, "peers not connected (call lqcd_slab_connect)");
+        if (need_gauge && !s->gauge_loaded) return fail(s, LQCD_ESTATE, "gauge field not loaded (call lqcd_slab_load_gauge)");
+        if (s->seq != G.s[0]->seq || s->recon != G.s[0]->recon || memcmp(s->L, G.s[0]->L, sizeof s->L))
+            return fail(s, LQCD_ESTATE, "the slabs of a group must share lattice, options and call history");
+    }
+    return LQCD_OK;
+}
+
+// One rank alone (n = 1 of a larger job): the group is that slab; its peers are other processes.
+int single_check(lqcd_slab* s, bool need_gauge)
+{
+    if (!s) return LQCD_EARG;
+    if (!s->memory_set) return fail(s, LQCD_ESTATE, "memory not set (call lqcd_slab_set_memory)");
+    if (!s->connected) return fail(s, LQCD_ESTATE, "peers not connected (call lqcd_slab_connect)");
+    if (need_gauge && !s->gauge_loaded) return fail(s, LQCD_ESTATE, "gauge field not loaded (call lqcd_slab_load_gauge)");
+    return LQCD_OK;
+}
+
+int use_device(lqcd_slab* s)
+{
+    SLAB_CUDA(cudaSetDevice(s->device));
+    return LQCD_OK;
+}
+
+// ---------------------------------------------------------------- pieces of a phase
+SlabPush push_next(const lqcd_slab* s)
+{
+    // faces stored now are read after the NEXT synchronisation point: buffer (seq + 1) & 1
+    const int buf = (int)((s->seq + 1) & 1ull);
+    const int R = s->nranks;
+    SlabPush ph;
+    ph.lo = s->ghost(s->peer[(s->rank + R - 1) % R], buf, 1);  // my first slice is the lower rank's "above"
+    ph.hi = s->ghost(s->peer[(s->rank + 1) % R], buf, 0);      // my last slice is the upper rank's "below"
+    ph.sh = s->sh;
+    ph.Vh = s->g.Vh;
+    return ph;
+}
+
+StagArgsD stag_args(const lqcd_slab* s, int parity, const cplx* in, cplx* out, bool push)
+{
+    StagArgsD a;
+    memset(&a, 0, sizeof a);
+    a.g = s->g;
+    a.parity = parity;
+    a.gauge = s->gauge();
+    a.in = in;
+    a.out = out;
+    a.sc = s->sc();
+    a.rs = s->rs();
+    a.hist = s->hist();
+    a.sl.t0 = s->t0;
+    a.sl.L3g = s->L[3];
+    a.sl.sh = s->sh;
+    const int buf = (int)(s->seq & 1ull);  // faces of `in` arrived with the last synchronisation point
+    a.sl.ghost_lo = s->ghost(s->mb, buf, 0);
+    a.sl.ghost_hi = s->ghost(s->mb, buf, 1);
+    a.sl.gauge_ghost = s->gghost();
+    if (push) {
+        const SlabPush ph = push_next(s);
+        a.sl.push_lo = ph.lo;
+        a.sl.push_hi = ph.hi;
+    }
+    a.sl.part = s->ss()->part;
+    return a;
+}
+
+template <int EPI>
+int launch_stag(lqcd_slab* s, const StagArgsD& a)
+{
+    const unsigned int grid = blocks_for(s->g.Vh, kStagBlock);
+    if (s->recon == 12)
+        stag_dslash_slab_kernel<EPI, kStagBlock, 12, cplx><<<grid, kStagBlock, 0, s->stream>>>(a);
+    else
+        stag_dslash_slab_kernel<EPI, kStagBlock, 18, cplx><<<grid, kStagBlock, 0, s->stream>>>(a);
+    SLAB_LAUNCH_CHECK();
+    return LQCD_OK;
+}
+
+int launch_push_faces(lqcd_slab* s, const cplx* v)
+{
+    const unsigned int grid = blocks_for(6 * (size_t)s->sh, kVecBlock);
+    slab_push_faces_kernel<kVecBlock><<<grid < 1184 ? grid : 1184, kVecBlock, 0, s->stream>>>(v, push_next(s));
+    SLAB_LAUNCH_CHECK();
+    return LQCD_OK;
+}
+
+SlabSyncArgs sync_args(const lqcd_slab* s, int op, int nvals, double m2, double tol, int maxiter)
+{
+    SlabSyncArgs a;
+    memset(&a, 0, sizeof a);
+    a.rank = s->rank;
+    a.nranks = s->nranks;
+    a.seq = s->seq;
+    a.nvals = nvals;
+    a.own.flag = (unsigned long long*)(s->mb + s->mb_flag);
+    a.own.slot = (double*)(s->mb + s->mb_slot);
+    a.own.ghost = (cplx*)(s->mb + s->mb_ghost);
+    for (int r = 0; r < s->nranks; ++r) {
+        a.peer_flag[r] = (unsigned long long*)(s->peer[r] + s->mb_flag);
+        a.peer_slot[r] = (double*)(s->peer[r] + s->mb_slot);
+    }
+    a.ss = s->ss();
+    a.sc = s->sc();
+    a.hist = s->hist();
+    a.op = op;
+    a.m2 = m2;
+    a.tol = tol;
+    a.maxiter = maxiter;
+    a.timeout_ns = (unsigned long long)s->timeout_ms * 1000000ull;
+    return a;
+}
+
+// One synchronisation point for the whole group: every slab signals, then every slab waits and
+// combines.  (With all slabs on one stream the signals therefore precede every wait: no kernel spins.)
+int group_sync(const Group& G, int op, int nvals, double m2 = 0.0, double tol = 0.0, int maxiter = 0)
+{
+    for (int r = 0; r < G.n; ++r) G.s[r]->seq += 1;
+    for (int r = 0; r < G.n; ++r) {
+        lqcd_slab* s = G.s[r];
+        int rc = use_device(s);
+        if (rc) return rc;
+        slab_signal_kernel<<<1, 32, 0, s->stream>>>(sync_args(s, op, nvals, m2, tol, maxiter));
+        SLAB_LAUNCH_CHECK();
+    }
+    for (int r = 0; r < G.n; ++r) {
+        lqcd_slab* s = G.s[r];
+        int rc = use_device(s);
+        if (rc) return rc;
+        slab_wait_combine_kernel<<<1, 32, 0, s->stream>>>(sync_args(s, op, nvals, m2, tol, maxiter));
+        SLAB_LAUNCH_CHECK();
+    }
+    return LQCD_OK;
+}
+
+int ensure_host(lqcd_slab* s)
+{
+    if (s->host_ready) return LQCD_OK;
+    SLAB_CUDA(cudaHostAlloc((void**)&s->h_sc, 2 * sizeof(CgScalars), cudaHostAllocDefault));
+    SLAB_CUDA(cudaHostAlloc((void**)&s->h_ss, sizeof(SlabScalars), cudaHostAllocDefault));
+    SLAB_CUDA(cudaEventCreateWithFlags(&s->ev[0], cudaEventDisableTiming));
+    SLAB_CUDA(cudaEventCreateWithFlags(&s->ev[1], cudaEventDisableTiming));
+    s->host_ready = true;
+    return LQCD_OK;
+}
+
+int read_scalars(lqcd_slab* s, int slot)
+{
+    SLAB_CUDA(cudaMemcpyAsync(&s->h_sc[slot], s->sc(), sizeof(CgScalars), cudaMemcpyDeviceToHost, s->stream));
+    SLAB_CUDA(cudaEventRecord(s->ev[slot], s->stream));
+    return LQCD_OK;
+}
+
+// Drain every slab's stream and report a timed-out wait.
+int group_finish(const Group& G)
+{
+    for (int r = 0; r < G.n; ++r) {
+        lqcd_slab* s = G.s[r];
+        int rc = use_device(s);
+        if (rc) return rc;
+        SLAB_CUDA(cudaMemcpyAsync(s->h_ss, s->ss(), sizeof(SlabScalars), cudaMemcpyDeviceToHost, s->stream));
+        SLAB_CUDA(cudaStreamSynchronize(s->stream));
+        if (s->h_ss->err) {
+            cudaMemsetAsync(&s->ss()->err, 0, sizeof(int), s->stream);
+            return fail(s, LQCD_ECOMM, "rank %d: a peer did not reach synchronisation point %llu within %d ms", s->rank,
+                        s->seq, s->timeout_ms);
+        }
+    }
+    return LQCD_OK;
+}
+
+// ---------------------------------------------------------------- operations on a group
+// Faces of a caller-supplied vector: a separate small kernel, then a synchronisation point.
+int group_halo_of(const Group& G, const cplx* const* v)
+{
+    for (int r = 0; r < G.n; ++r) {
+        int rc = use_device(G.s[r]);
+        if (rc) return rc;
+        rc = launch_push_faces(G.s[r], v[r]);
+        if (rc) return rc;
+    }
+    return group_sync(G, SLAB_OP_NONE, 0);
+}
+
+int group_dslash(const Group& G, int out_parity, const cplx* const* in, cplx* const* out)
+{
+    int rc = group_halo_of(G, in);
+    if (rc) return rc;
+    for (int r = 0; r < G.n; ++r) {
+        rc = use_device(G.s[r]);
+        if (rc) return rc;
+        rc = launch_stag<SE_PLAIN>(G.s[r], stag_args(G.s[r], out_parity, in[r], out[r], false));
+        if (rc) return rc;
+    }
+    return LQCD_OK;
+}
+
+// t = D_oe v with the faces of t pushed, then a halo-only synchronisation point: t is ready for D_eo.
+int group_first_hop(const Group& G, const cplx* const* v)
+{
+    int rc = group_halo_of(G, v);
+    if (rc) return rc;
+    for (int r = 0; r < G.n; ++r) {
+        rc = use_device(G.s[r]);
+        if (rc) return rc;
+        rc = launch_stag<SE_PLAIN>(G.s[r], stag_args(G.s[r], LQCD_ODD, v[r], G.s[r]->t(), true));
+        if (rc) return rc;
+    }
+    return group_sync(G, SLAB_OP_NONE, 0);
+}
+
+int group_MdagM(const Group& G, double mass, const cplx* const* in, cplx* const* out)
+{
+    int rc = group_first_hop(G, in);
+    if (rc) return rc;
+    for (int r = 0; r < G.n; ++r) {
+        lqcd_slab* s = G.s[r];
+        rc = use_device(s);
+        if (rc) return rc;
+        StagArgsD a = stag_args(s, LQCD_EVEN, s->t(), out[r], false);
+        a.m2 = mass * mass;
+        a.p = in[r];
+        rc = launch_stag<SE_MDAGM>(s, a);
+        if (rc) return rc;
+    }
+    return LQCD_OK;
+}
+
+// One CG iteration (S1-S5) = three producer phases, each closed by a synchronisation point.
+int group_iteration(const Group& G, double mass, cplx* const* x)
+{
+    const double m2 = mass * mass;
+    int rc;
+    for (int r = 0; r < G.n; ++r) {  // S1: t = D_oe p, partial <t,t>; faces of t -> neighbours
+        lqcd_slab* s = G.s[r];
+        rc = use_device(s);
+        if (rc) return rc;
+        rc = launch_stag<SE_NORM>(s, stag_args(s, LQCD_ODD, s->p(), s->t(), true));
+        if (rc) return rc;
+    }
+    rc = group_sync(G, SLAB_OP_ALPHA, 1, m2);  // S2
+    if (rc) return rc;
+    for (int r = 0; r < G.n; ++r) {  // S3: D_eo t fused with the x / r updates, partial <r,r>
+        lqcd_slab* s = G.s[r];
+        rc = use_device(s);
+        if (rc) return rc;
+        StagArgsD a = stag_args(s, LQCD_EVEN, s->t(), nullptr, false);
+        a.m2 = m2;
+        a.p = s->p();
+        a.x = x[r];
+        a.r = s->r();
+        rc = launch_stag<SE_CGUPDATE>(s, a);
+        if (rc) return rc;
+    }
+    rc = group_sync(G, SLAB_OP_UPDATE, 1);  // beta, exit test (S4 happens on every rank identically)
+    if (rc) return rc;
+    for (int r = 0; r < G.n; ++r) {  // S5: p = r + beta p, partial <p,p>; faces of p -> neighbours
+        lqcd_slab* s = G.s[r];
+        rc = use_device(s);
+        if (rc) return rc;
+        slab_cg_pupdate_kernel<kVecBlock><<<vec_grid(s), kVecBlock, 0, s->stream>>>(s->r(), s->p(), s->nvec, push_next(s),
+                                                                                   s->sc(), s->ss(), s->rs());
+        SLAB_LAUNCH_CHECK();
+    }
+    return group_sync(G, SLAB_OP_PP, 1);
+}
+
+int group_cg(const Group& G, double mass, double tol, int maxiter, const cplx* const* b, cplx* const* x, int* iters,
+             double* true_residual)
+{
+    int rc;
+    lqcd_slab* s0 = G.s[0];
+    for (int r = 0; r < G.n; ++r) {  // S6
+        lqcd_slab* s = G.s[r];
+        rc = use_device(s);
+        if (rc) return rc;
+        slab_cg_init_kernel<kVecBlock><<<vec_grid(s), kVecBlock, 0, s->stream>>>(b[r], x[r], s->r(), s->p(), s->nvec,
+                                                                                push_next(s), s->ss(), s->rs());
+        SLAB_LAUNCH_CHECK();
+    }
+    rc = group_sync(G, SLAB_OP_INIT, 1, 0.0, tol, maxiter);
+    if (rc) return rc;
+
+    // Host loop as LQCD_CG_ASYNC of lqcd_cg_solve: batches of check_every iterations are enqueued
+    // while the previous batch's scalars travel; after `done` every kernel of every rank is a no-op
+    // (signals and waits still run, so the ranks stay in step).  The scalars are bit-identical on all
+    // ranks; rank 0's copy (of this process) is the one read.
+    CgScalars* h = s0->h_sc;
+    const int batch = s0->check_every;
+    int slot = 0;
+    bool pending[2] = { false, false };
+    bool finished = false;
+    long long enqueued = 0;
+    while (!finished) {
+        if (enqueued < (long long)maxiter) {
+            for (int k = 0; k < batch; ++k) {
+                rc = group_iteration(G, mass, x);
+                if (rc) return rc;
+            }
+            enqueued += batch;
+        }
+        rc = use_device(s0);
+        if (rc) return rc;
+        rc = read_scalars(s0, slot);
+        if (rc) return rc;
+        pending[slot] = true;
+        const int other = slot ^ 1;
+        if (pending[other]) {
+            lqcd_slab* s = s0;
+            SLAB_CUDA(cudaEventSynchronize(s->ev[other]));
+            pending[other] = false;
+            if (h[other].done) finished = true;
+        }
+        slot = other;
+    }
+    rc = group_finish(G);
+    if (rc) return rc;
+
+    // S7: |b - A x| / |b| with a fresh A
+    rc = group_first_hop(G, x);
+    if (rc) return rc;
+    for (int r = 0; r < G.n; ++r) {
+        lqcd_slab* s = G.s[r];
+        rc = use_device(s);
+        if (rc) return rc;
+        StagArgsD a = stag_args(s, LQCD_EVEN, s->t(), nullptr, false);
+        a.m2 = mass * mass;
+        a.p = x[r];
+        a.b = b[r];
+        rc = launch_stag<SE_RESIDUAL>(s, a);
+        if (rc) return rc;
+    }
+    rc = group_sync(G, SLAB_OP_RES2, 1);
+    if (rc) return rc;
+    rc = use_device(s0);
+    if (rc) return rc;
+    rc = read_scalars(s0, 0);
+    if (rc) return rc;
+    rc = group_finish(G);
+    if (rc) return rc;
+    *iters = h[0].iter;
+    *true_residual = h[0].bb > 0.0 ? sqrt(h[0].res2 / h[0].bb) : 0.0;
+    return h[0].rr_new <= h[0].thresh ? LQCD_OK : LQCD_MAXITER;
+}
+
+}  // namespace
+
+// =========================================================================== C-ABI
+extern "C" {
+
+int lqcd_slab_create(lqcd_slab** out, int L0, int L1, int L2, int L3, int rank, int nranks)
+{
+    if (!out) return LQCD_EARG;
+    *out = nullptr;
+    if (nranks < 1 || nranks > LQCD_SLAB_MAX_RANKS || rank < 0 || rank >= nranks) return LQCD_EARG;
+    const int L[4] = { L0, L1, L2, L3 };
+    for (int mu = 0; mu < 4; ++mu)
+        if (L[mu] < 2 || (L[mu] & 1)) return LQCD_EDIM;
+    if (L3 % nranks) return LQCD_EDIM;
+    const int T = L3 / nranks;
+    if (T < 2 || (T & 1)) return LQCD_EDIM;  // even slabs keep local parity = global parity
+    const long long V = (long long)L0 * L1 * L2 * T;
+    if (V > (1LL << 30)) return LQCD_EDIM;
+    lqcd_slab* c = (lqcd_slab*)calloc(1, sizeof(lqcd_slab));
+    if (!c) return LQCD_ENOMEM;
+    memcpy(c->L, L, sizeof L);
+    c->rank = rank;
+    c->nranks = nranks;
+    c->T = T;
+    c->t0 = rank * T;
+    c->g.Lh = L0 / 2;
+    c->g.L1 = L1;
+    c->g.L2 = L2;
+    c->g.L3 = T;
+    c->g.s1 = c->g.Lh;
+    c->g.s2 = c->g.Lh * L1;
+    c->g.s3 = c->g.Lh * L1 * L2;
+    c->g.V = V;
+    c->g.Vh = (int)(V / 2);
+    c->sh = c->g.s3;
+    c->nvec = 3 * (size_t)(V / 2);
+    c->max_blocks = (size_t)V / 64 + 4096;
+    c->recon = 18;
+    c->check_every = 8;
+    c->timeout_ms = 20000;
+
+    size_t off = 0;
+    const size_t vec_bytes = align_up(c->nvec * sizeof(cplx));
+    c->off_gauge = off;     off += align_up((size_t)V * 36 * sizeof(cplx));
+    c->off_gghost = off;    off += align_up(2 * 9 * (size_t)c->sh * sizeof(cplx));
+    c->off_r = off;         off += vec_bytes;
+    c->off_p = off;         off += vec_bytes;
+    c->off_t = off;         off += vec_bytes;
+    c->off_sc = off;        off += align_up(sizeof(CgScalars));
+    c->off_ss = off;        off += align_up(sizeof(SlabScalars));
+    c->off_ticket = off;    off += kAlign;
+    c->off_partials = off;  off += align_up(c->max_blocks * sizeof(double));
+    c->off_hist = off;      off += align_up((size_t)kHistCap * sizeof(double));
+    c->ws_needed = off;
+
+    off = 0;
+    c->mb_flag = off;   off += align_up(LQCD_SLAB_MAX_RANKS * sizeof(unsigned long long));
+    c->mb_slot = off;   off += align_up(2 * LQCD_SLAB_MAX_RANKS * 2 * sizeof(double));
+    c->mb_ghost = off;  off += align_up(2 * 2 * 3 * (size_t)c->sh * sizeof(cplx));
+    c->mb_needed = off;
+    *out = c;
+    return LQCD_OK;
+}
+
+int lqcd_slab_destroy(lqcd_slab* s)
+{
+    if (!s) return LQCD_EARG;
+    if (s->host_ready) {
+        cudaFreeHost(s->h_sc);
+        cudaFreeHost(s->h_ss);
+        cudaEventDestroy(s->ev[0]);
+        cudaEventDestroy(s->ev[1]);
+    }
+    free(s);
+    return LQCD_OK;
+}
+
+size_t lqcd_slab_workspace_bytes(const lqcd_slab* s) { return s ? s->ws_needed : 0; }
+size_t lqcd_slab_mailbox_bytes(const lqcd_slab* s) { return s ? s->mb_needed : 0; }
+
+int lqcd_slab_set_memory(lqcd_slab* s, void* workspace_dev, size_t workspace_bytes, void* mailbox_dev, size_t mailbox_bytes,
+                         void* cuda_stream)
+{
+    if (!s) return LQCD_EARG;
+    if (!workspace_dev || !mailbox_dev) return fail(s, LQCD_EARG, "null workspace or mailbox pointer");
+    if (((uintptr_t)workspace_dev) % kAlign || ((uintptr_t)mailbox_dev) % kAlign)
+        return fail(s, LQCD_EARG, "workspace and mailbox must be 256-byte aligned");
+    if (workspace_bytes < s->ws_needed)
+        return fail(s, LQCD_ENOMEM, "workspace too small: %zu bytes given, %zu needed", workspace_bytes, s->ws_needed);
+    if (mailbox_bytes < s->mb_needed)
+        return fail(s, LQCD_ENOMEM, "mailbox too small: %zu bytes given, %zu needed", mailbox_bytes, s->mb_needed);
+    int ndev = 0;
+    SLAB_CUDA(cudaGetDeviceCount(&ndev));
+    if (ndev < 1) return fail(s, LQCD_ECUDA, "no CUDA device");
+    cudaPointerAttributes at;
+    SLAB_CUDA(cudaPointerGetAttributes(&at, workspace_dev));
+    if (at.type != cudaMemoryTypeDevice) return fail(s, LQCD_EARG, "workspace is not device memory");
+    s->device = at.device;
+    SLAB_CUDA(cudaSetDevice(s->device));
+    int rc = ensure_host(s);
+    if (rc) return rc;
+    s->ws = (char*)workspace_dev;
+    s->mb = (char*)mailbox_dev;
+    s->stream = (cudaStream_t)cuda_stream;
+    s->memory_set = true;
+    s->connected = false;
+    s->gauge_loaded = false;
+    s->seq = 0;
+    SLAB_CUDA(cudaMemsetAsync(s->ws + s->off_sc, 0, align_up(sizeof(CgScalars)) + align_up(sizeof(SlabScalars)) + kAlign, s->stream));
+    SLAB_CUDA(cudaMemsetAsync(s->mb, 0, s->mb_ghost, s->stream));  // flags and slots
+    SLAB_CUDA(cudaStreamSynchronize(s->stream));
+    return LQCD_OK;
+}
+
+int lqcd_slab_connect(lqcd_slab* s, void* const* peer_mailboxes)
+{
+    if (!s) return LQCD_EARG;
+    if (!s->memory_set) return fail(s, LQCD_ESTATE, "memory not set (call lqcd_slab_set_memory)");
+    if (!peer_mailboxes) return fail(s, LQCD_EARG, "peer_mailboxes is null");
+    for (int r = 0; r < s->nranks; ++r)
+        if (!peer_mailboxes[r]) return fail(s, LQCD_EARG, "mailbox of rank %d is null", r);
+    if (peer_mailboxes[s->rank] != (void*)s->mb) return fail(s, LQCD_EARG, "peer_mailboxes[rank] must be the own mailbox");
+    for (int r = 0; r < s->nranks; ++r) s->peer[r] = (char*)peer_mailboxes[r];
+    s->connected = true;
+    return LQCD_OK;
+}
+
+int lqcd_slab_set_option(lqcd_slab* s, int option, int value)
+{
+    if (!s) return LQCD_EARG;
+    if (option == LQCD_SLAB_OPT_RECONSTRUCT) {
+        if (value != 18 && value != 12) return fail(s, LQCD_EARG, "reconstruct must be 18 or 12");
+        if (value != s->recon) s->gauge_loaded = false;
+        s->recon = value;
+        return LQCD_OK;
+    }
+    if (option == LQCD_SLAB_OPT_CHECK_EVERY) {
+        if (value < 1 || value > 1024) return fail(s, LQCD_EARG, "check_every must be in 1..1024");
+        s->check_every = value;
+        return LQCD_OK;
+    }
+    if (option == LQCD_SLAB_OPT_TIMEOUT_MS) {
+        if (value < 1 || value > 600000) return fail(s, LQCD_EARG, "timeout must be in 1..600000 ms");
+        s->timeout_ms = value;
+        return LQCD_OK;
+    }
+    return fail(s, LQCD_EARG, "unknown option %d", option);
+}
+
+int lqcd_slab_load_gauge(lqcd_slab* s, const double* u_local_dev, const double* u3_below_dev)
+{
+    if (!s) return LQCD_EARG;
+    if (!s->memory_set) return fail(s, LQCD_ESTATE, "memory not set (call lqcd_slab_set_memory)");
+    if (!u_local_dev || !u3_below_dev) return fail(s, LQCD_EARG, "null gauge pointer");
+    SLAB_CUDA(cudaSetDevice(s->device));
+    const size_t V = (size_t)s->g.V;
+    const unsigned int grid = blocks_for(V, kReorderTile);
+    const unsigned int ggrid = blocks_for(18 * (size_t)s->sh, 256);
+    if (s->recon == 12) {
+        gauge_reorder_kernel<256, kReorderTile, 12, cplx><<<grid, 256, 0, s->stream>>>((const cplx*)u_local_dev, s->gauge(),
+                                                                                       (size_t)s->g.Vh);
+        SLAB_LAUNCH_CHECK();
+        slab_ghost_links_kernel<12><<<ggrid, 256, 0, s->stream>>>((const cplx*)u3_below_dev, s->gghost(), (size_t)s->sh);
+    } else {
+        gauge_reorder_kernel<256, kReorderTile, 18, cplx><<<grid, 256, 0, s->stream>>>((const cplx*)u_local_dev, s->gauge(),
+                                                                                       (size_t)s->g.Vh);
+        SLAB_LAUNCH_CHECK();
+        slab_ghost_links_kernel<18><<<ggrid, 256, 0, s->stream>>>((const cplx*)u3_below_dev, s->gghost(), (size_t)s->sh);
+    }
+    SLAB_LAUNCH_CHECK();
+    s->gauge_loaded = true;
+    return LQCD_OK;
+}
+
+// ---- group calls
+int lqcd_slab_dslash_group(lqcd_slab* const* slabs, int n, int out_parity, const double* const* in_dev, double* const* out_dev)
+{
+    const Group G = { slabs, n };
+    int rc = group_check(G, true);
+    if (rc) return rc;
+    lqcd_slab* s = slabs[0];
+    if (!in_dev || !out_dev) return fail(s, LQCD_EARG, "null pointer array");
+    if (out_parity != LQCD_EVEN && out_parity != LQCD_ODD) return fail(s, LQCD_EARG, "bad parity %d", out_parity);
+    for (int r = 0; r < n; ++r)
+        if (!in_dev[r] || !out_dev[r] || in_dev[r] == out_dev[r]) return fail(s, LQCD_EARG, "null or aliased vector of rank %d", r);
+    return group_dslash(G, out_parity, (const cplx* const*)in_dev, (cplx* const*)out_dev);
+}
+
+int lqcd_slab_apply_MdagM_group(lqcd_slab* const* slabs, int n, double mass, const double* const* in_dev, double* const* out_dev)
+{
+    const Group G = { slabs, n };
+    int rc = group_check(G, true);
+    if (rc) return rc;
+    lqcd_slab* s = slabs[0];
+    if (!in_dev || !out_dev) return fail(s, LQCD_EARG, "null pointer array");
+    for (int r = 0; r < n; ++r)
+        if (!in_dev[r] || !out_dev[r] || in_dev[r] == out_dev[r]) return fail(s, LQCD_EARG, "null or aliased vector of rank %d", r);
+    return group_MdagM(G, mass, (const cplx* const*)in_dev, (cplx* const*)out_dev);
+}
+
+int lqcd_slab_cg_solve_group(lqcd_slab* const* slabs, int n, double mass, double tol, int maxiter, const double* const* b_dev,
+                             double* const* x_dev, int* iters, double* true_residual)
+{
+    const Group G = { slabs, n };
+    int rc = group_check(G, true);
+    if (rc) return rc;
+    lqcd_slab* s = slabs[0];
+    if (!b_dev || !x_dev || !iters || !true_residual) return fail(s, LQCD_EARG, "null pointer argument");
+    if (!(tol >= 0.0) || maxiter < 0) return fail(s, LQCD_EARG, "tol must be >= 0 and maxiter >= 0");
+    for (int r = 0; r < n; ++r)
+        if (!b_dev[r] || !x_dev[r] || b_dev[r] == x_dev[r]) return fail(s, LQCD_EARG, "null or aliased vector of rank %d", r);
+    return group_cg(G, mass, tol, maxiter, (const cplx* const*)b_dev, (cplx* const*)x_dev, iters, true_residual);
+}
+
+// ---- one rank per process: the n = 1 group whose peers live elsewhere
+int lqcd_slab_dslash(lqcd_slab* s, int out_parity, const double* in_dev, double* out_dev)
+{
+    int rc = single_check(s, true);
+    if (rc) return rc;
+    if (!in_dev || !out_dev || in_dev == out_dev) return fail(s, LQCD_EARG, "null or aliased vector");
+    if (out_parity != LQCD_EVEN && out_parity != LQCD_ODD) return fail(s, LQCD_EARG, "bad parity %d", out_parity);
+    lqcd_slab* one[1] = { s };
+    const Group G = { one, 1 };
+    const cplx* in[1] = { (const cplx*)in_dev };
+    cplx* out[1] = { (cplx*)out_dev };
+    return group_dslash(G, out_parity, in, out);
+}
+
+int lqcd_slab_apply_MdagM(lqcd_slab* s, double mass, const double* in_dev, double* out_dev)
+{
+    int rc = single_check(s, true);
+    if (rc) return rc;
+    if (!in_dev || !out_dev || in_dev == out_dev) return fail(s, LQCD_EARG, "null or aliased vector");
+    lqcd_slab* one[1] = { s };
+    const Group G = { one, 1 };
+    const cplx* in[1] = { (const cplx*)in_dev };
+    cplx* out[1] = { (cplx*)out_dev };
+    return group_MdagM(G, mass, in, out);
+}
+
+int lqcd_slab_cg_solve(lqcd_slab* s, double mass, double tol, int maxiter, const double* b_dev, double* x_dev, int* iters,
+                       double* true_residual)
+{
+    int rc = single_check(s, true);
+    if (rc) return rc;
+    if (!b_dev || !x_dev || !iters || !true_residual || b_dev == x_dev) return fail(s, LQCD_EARG, "null or aliased argument");
+    if (!(tol >= 0.0) || maxiter < 0) return fail(s, LQCD_EARG, "tol must be >= 0 and maxiter >= 0");
+    lqcd_slab* one[1] = { s };
+    const Group G = { one, 1 };
+    const cplx* b[1] = { (const cplx*)b_dev };
+    cplx* x[1] = { (cplx*)x_dev };
+    return group_cg(G, mass, tol, maxiter, b, x, iters, true_residual);
+}
+
+// ---- CUDA IPC: mailboxes across processes
+int lqcd_slab_ipc_export(lqcd_slab* s, unsigned char handle[64], size_t* offset)
+{
+    if (!s) return LQCD_EARG;
+    if (!s->memory_set) return fail(s, LQCD_ESTATE, "memory not set (call lqcd_slab_set_memory)");
+    if (!handle || !offset) return fail(s, LQCD_EARG, "null pointer argument");
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "the ABI carries IPC handles as 64 bytes");
+    SLAB_CUDA(cudaSetDevice(s->device));
+    // the handle names the whole allocation the mailbox lies in; find its base through the driver
+    typedef int (*AddressRangeFn)(unsigned long long*, size_t*, unsigned long long);
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    SLAB_CUDA(cudaGetDriverEntryPoint("cuMemGetAddressRange", &fn, cudaEnableDefault, &q));
+    if (!fn || q != cudaDriverEntryPointSuccess) return fail(s, LQCD_ECUDA, "cuMemGetAddressRange is not available");
+    unsigned long long base = 0;
+    size_t size = 0;
+    const int cr = ((AddressRangeFn)fn)(&base, &size, (unsigned long long)(uintptr_t)s->mb);
+    if (cr != 0) return fail(s, LQCD_ECUDA, "cuMemGetAddressRange failed with CUresult %d", cr);
+    cudaIpcMemHandle_t h;
+    SLAB_CUDA(cudaIpcGetMemHandle(&h, (void*)(uintptr_t)base));
+    memcpy(handle, &h, 64);
+    *offset = (size_t)((unsigned long long)(uintptr_t)s->mb - base);
+    return LQCD_OK;
+}
+
+int lqcd_slab_ipc_open(lqcd_slab* s, const unsigned char handle[64], size_t offset, void** peer_mailbox)
+{
+    if (!s) return LQCD_EARG;
+    if (!handle || !peer_mailbox) return fail(s, LQCD_EARG, "null pointer argument");
+    if (!s->memory_set) return fail(s, LQCD_ESTATE, "memory not set (call lqcd_slab_set_memory)");
+    SLAB_CUDA(cudaSetDevice(s->device));
+    cudaIpcMemHandle_t h;
+    memcpy(&h, handle, 64);
+    void* base = nullptr;
+    SLAB_CUDA(cudaIpcOpenMemHandle(&base, h, cudaIpcMemLazyEnablePeerAccess));
+    *peer_mailbox = (char*)base + offset;
+    return LQCD_OK;
+}
+
+int lqcd_slab_ipc_close(lqcd_slab* s, void* peer_mailbox, size_t offset)
+{
+    if (!s) return LQCD_EARG;
+    if (!peer_mailbox) return fail(s, LQCD_EARG, "null pointer argument");
+    SLAB_CUDA(cudaIpcCloseMemHandle((char*)peer_mailbox - offset));
+    return LQCD_OK;
+}
+
+long long lqcd_slab_sync_points(const lqcd_slab* s) { return s ? (long long)s->seq : 0; }
+long long lqcd_slab_kernel_launches(const lqcd_slab* s) { return s ? s->launches : 0; }
+const char* lqcd_slab_last_error(const lqcd_slab* s) { return s ? s->err : "null slab"; }
+
+}  // extern "C"

@@ -33,6 +33,22 @@ enum StagEpilogue {
     SE_RELIABLE = 9         // fp64: r = b - (m^2 p - D in), rf = fl32(r), |r|^2; resumes the paused iteration
 };
 
+// Time-slab decomposition (include/lqcd_slab.h).  The Geom of a slab is
+// that of its local L0 x L1 x L2 x T lattice; hops in time that leave the slab read the neighbour
+// rank's boundary time-slice from a ghost face ([3][sh], sh = sites of one parity in a time-slice)
+// that the neighbour's producing kernel stored there through peer memory, and the backward hop at
+// the first local slice reads U_3 of the slice below from a ghost copy ([parity][NC][sh]).
+template <class C>
+struct SlabArgs {
+    int t0, L3g, sh;       // first global time-slice of the slab, global time extent, half-slice sites
+    const C* ghost_lo;     // input vector on time-slice t0-1 (global, periodic), parity of `in`
+    const C* ghost_hi;     // input vector on time-slice t0+T
+    const C* gauge_ghost;  // U_3 on time-slice t0-1
+    C* push_lo;            // where the slab below (rank-1) keeps its ghost_hi: receives `out` on local slice 0
+    C* push_hi;            // where the slab above (rank+1) keeps its ghost_lo: receives `out` on local slice T-1
+    double* part;          // this rank's partial sums (the cross-rank combine kernel adds them in rank order)
+};
+
 template <class C>
 struct StagArgs {
     Geom g;
@@ -50,31 +66,62 @@ struct StagArgs {
     CgScalars* sc;
     ReduceScratch rs;
     double* hist;
+    SlabArgs<C> sl;  // used by the SLAB instantiations only
 };
 
-template <int MU, int RECON, class C>
+template <int MU, int RECON, bool SLAB, class C>
 __device__ __forceinline__ void stag_hop(const StagArgs<C>& a, const Site& s, C acc[3])
 {
     constexpr int NC = RECON / 2;
     const size_t Vh = (size_t)a.g.Vh;
     const double eta = half_eta<MU>(s);
-    const int ef = nbr_fwd<MU>(a.g, s);
-    const int eb = nbr_bwd<MU>(a.g, s);
     const C* Uf = a.gauge + (size_t)((a.parity * 4 + MU) * NC) * Vh + s.e;
-    const C* Ub = a.gauge + (size_t)(((1 - a.parity) * 4 + MU) * NC) * Vh + eb;
-
     C U[9], W[9], vf[3], vb[3];
-    load_link<RECON>(Uf, Vh, U);
+    double sf, sb;
+    if (SLAB && MU == 3) {
+        // time hops of a slab: no wrap inside the slab; the two boundary slices read the ghost faces
+        // (written by the neighbour ranks through peer memory: L2 loads, never the read-only path)
+        const bool top = s.x3 + 1 == a.g.L3, bottom = s.x3 == 0;
+        const size_t sh = (size_t)a.sl.sh;
+        load_link<RECON>(Uf, Vh, U);
+        if (top) {
+            const C* v = a.sl.ghost_hi + (s.e - (a.g.L3 - 1) * a.g.s3);
 #pragma unroll
-    for (int c = 0; c < 3; ++c) vf[c] = ld_keep(a.in + c * Vh + ef);
-    load_link<RECON>(Ub, Vh, W);
+            for (int c = 0; c < 3; ++c) vf[c] = __ldcg(v + c * sh);
+        } else {
 #pragma unroll
-    for (int c = 0; c < 3; ++c) vb[c] = ld_keep(a.in + c * Vh + eb);
+            for (int c = 0; c < 3; ++c) vf[c] = ld_keep(a.in + c * Vh + s.e + a.g.s3);
+        }
+        if (bottom) {
+            load_link<RECON>(a.sl.gauge_ghost + (size_t)((1 - a.parity) * NC) * sh + s.e, sh, W);
+            const C* v = a.sl.ghost_lo + s.e;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) vb[c] = __ldcg(v + c * sh);
+        } else {
+            const int eb = s.e - a.g.s3;
+            load_link<RECON>(a.gauge + (size_t)(((1 - a.parity) * 4 + MU) * NC) * Vh + eb, Vh, W);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) vb[c] = ld_keep(a.in + c * Vh + eb);
+        }
+        // antiperiodic boundary of the GLOBAL lattice (reading A4)
+        sf = (a.sl.t0 + s.x3 + 1 == a.sl.L3g) ? -eta : eta;
+        sb = (a.sl.t0 + s.x3 == 0) ? eta : -eta;
+    } else {
+        const int ef = nbr_fwd<MU>(a.g, s);
+        const int eb = nbr_bwd<MU>(a.g, s);
+        const C* Ub = a.gauge + (size_t)(((1 - a.parity) * 4 + MU) * NC) * Vh + eb;
+        load_link<RECON>(Uf, Vh, U);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) vf[c] = ld_keep(a.in + c * Vh + ef);
+        load_link<RECON>(Ub, Vh, W);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) vb[c] = ld_keep(a.in + c * Vh + eb);
+        sf = eta * bc_fwd<MU>(a.g, s);
+        sb = -eta * bc_bwd<MU>(a.g, s);
+    }
     reconstruct_link<RECON>(U);
     reconstruct_link<RECON>(W);
 
-    const double sf = eta * bc_fwd<MU>(a.g, s);
-    const double sb = -eta * bc_bwd<MU>(a.g, s);
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         vf[c] = cscale(sf, vf[c]);
@@ -114,8 +161,27 @@ __device__ __forceinline__ void stag_hop(const StagArgs<C>& a, const Site& s, C 
 template <int RECON, class C> struct StagMinBlocks { static constexpr int value = RECON == 12 ? LQCD_STAG_MINB12 : LQCD_STAG_MINB18; };
 template <int RECON> struct StagMinBlocks<RECON, cplxf> { static constexpr int value = RECON == 12 ? LQCD_STAG_MINB12F : LQCD_STAG_MINB18F; };
 
-template <int EPI, int BLOCK, int RECON, class C>
-__global__ void __launch_bounds__(BLOCK, StagMinBlocks<RECON, C>::value) stag_dslash_kernel(const StagArgs<C> a)
+// Slab kernels that produce a vector the next Dslash will read (SE_PLAIN, SE_NORM) also store its
+// two boundary time-slices into the neighbour ranks' ghost faces: the halo exchange is part of the
+// producing kernel (stores through peer memory over NVLink), not a separate pack + send.
+template <class C>
+__device__ __forceinline__ void slab_push(const StagArgs<C>& a, int x3, int e, const C v[3])
+{
+    const size_t sh = (size_t)a.sl.sh;
+    if (a.sl.push_lo == nullptr) return;  // the vector produced is not the input of a later Dslash
+    if (x3 == 0) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) a.sl.push_lo[c * sh + e] = v[c];
+    }
+    if (x3 + 1 == a.g.L3) {
+        const int f = e - (a.g.L3 - 1) * a.g.s3;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) a.sl.push_hi[c * sh + f] = v[c];
+    }
+}
+
+template <int EPI, int BLOCK, int RECON, bool SLAB, class C>
+__device__ __forceinline__ void stag_dslash_body(const StagArgs<C>& a)
 {
     if (EPI == SE_NORM || EPI == SE_CGUPDATE || EPI == SE_CGUPDATE_MIXED) {
         // converged earlier, or waiting for a reliable update: this (pre-enqueued) iteration is a no-op
@@ -125,12 +191,60 @@ __global__ void __launch_bounds__(BLOCK, StagMinBlocks<RECON, C>::value) stag_ds
     const bool active = e < a.g.Vh;
     const size_t Vh = (size_t)a.g.Vh;
     C acc[3] = { czero<C>(), czero<C>(), czero<C>() };
+    int x3 = 0;
     if (active) {
         const Site s = decode_site(a.g, a.parity, e);
-        stag_hop<0, RECON>(a, s, acc);
-        stag_hop<1, RECON>(a, s, acc);
-        stag_hop<2, RECON>(a, s, acc);
-        stag_hop<3, RECON>(a, s, acc);
+        x3 = s.x3;
+        stag_hop<0, RECON, SLAB>(a, s, acc);
+        stag_hop<1, RECON, SLAB>(a, s, acc);
+        stag_hop<2, RECON, SLAB>(a, s, acc);
+        stag_hop<3, RECON, SLAB>(a, s, acc);
+    }
+    if (SLAB && (EPI == SE_PLAIN || EPI == SE_NORM)) {
+        if (active) slab_push(a, x3, e, acc);
+    }
+    if (SLAB && EPI != SE_PLAIN && EPI != SE_MDAGM) {
+        // Slab epilogues with a sum: the same per-site arithmetic as below, but the total over this
+        // rank's sites is only a partial; the scalar step runs in the cross-rank combine kernel.
+        double local = 0.0;
+        if (active) {
+            if (EPI == SE_NORM) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    st_vec(a.out + c * Vh + e, acc[c]);
+                    local += cnorm2(acc[c]);
+                }
+            } else if (EPI == SE_CGUPDATE) {
+                const double alpha = a.sc->alpha;
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const size_t i = c * Vh + e;
+                    const double2 pv = to_d(a.p[i]), q = to_d(acc[c]);
+                    double2 xv = to_d(a.x[i]), rv = to_d(a.r[i]);
+                    const double2 ap = cmake(fma(a.m2, pv.x, -q.x), fma(a.m2, pv.y, -q.y));
+                    xv.x = fma(alpha, pv.x, xv.x);
+                    xv.y = fma(alpha, pv.y, xv.y);
+                    rv.x = fma(-alpha, ap.x, rv.x);
+                    rv.y = fma(-alpha, ap.y, rv.y);
+                    const C rs_ = to_cplx(rv, (C*)0);
+                    a.x[i] = to_cplx(xv, (C*)0);
+                    a.r[i] = rs_;
+                    local += cnorm2(rs_);
+                }
+            } else {  // SE_RESIDUAL
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const size_t i = c * Vh + e;
+                    const double2 xv = to_d(a.p[i]), bv = to_d(a.b[i]), q = to_d(acc[c]);
+                    const double re = bv.x - fma(a.m2, xv.x, -q.x);
+                    const double im = bv.y - fma(a.m2, xv.y, -q.y);
+                    local += fma(re, re, im * im);
+                }
+            }
+        }
+        double* part = a.sl.part;
+        grid_sum<BLOCK>(local, a.rs, [part](double v) { part[0] = v; });
+        return;
     }
     if (EPI == SE_PLAIN) {
         if (active) {
@@ -245,6 +359,19 @@ __global__ void __launch_bounds__(BLOCK, StagMinBlocks<RECON, C>::value) stag_ds
         CgScalars* sc = a.sc;
         grid_sum<BLOCK>(local, a.rs, [sc](double res2) { sc->res2 = res2; });
     }
+}
+
+template <int EPI, int BLOCK, int RECON, class C>
+__global__ void __launch_bounds__(BLOCK, StagMinBlocks<RECON, C>::value) stag_dslash_kernel(const StagArgs<C> a)
+{
+    stag_dslash_body<EPI, BLOCK, RECON, false>(a);
+}
+
+// The same hopping term on one rank's time-slab (fp64; SE_PLAIN, SE_NORM, SE_MDAGM, SE_CGUPDATE, SE_RESIDUAL).
+template <int EPI, int BLOCK, int RECON, class C>
+__global__ void __launch_bounds__(BLOCK, StagMinBlocks<RECON, C>::value) stag_dslash_slab_kernel(const StagArgs<C> a)
+{
+    stag_dslash_body<EPI, BLOCK, RECON, true>(a);
 }
 
 }  // namespace lqcd

@@ -1,0 +1,220 @@
+"""Time-slab decomposition against the oracle of the GLOBAL lattice.
+
+The R slabs of a lattice are driven on the one GPU of the test box through the *_group calls of
+include/lqcd_slab.h: the kernels, the peer stores into the neighbours' ghost faces, the slot / flag
+mailboxes and the rank-ordered sums are those of an R-GPU run; all slabs share one stream, so no
+kernel ever waits for another (B200_PROFILING.md).  The decomposition must not change the
+mathematics: the assembled result is compared with the oracle on the undivided lattice at the
+north-star tolerances (Dslash 1e-13, CG 1e-9 and +-2 iterations)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_1311_2719_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+DSLASH_TOL = 1e-13
+CG_TOL = 1e-9
+
+
+@pytest.fixture(scope="module")
+def sl():
+    from paper_1311_2719_b200 import slab
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return slab
+
+
+def rel(a, b):
+    return np.linalg.norm((a - b).ravel()) / max(np.linalg.norm(b.ravel()), 1e-300)
+
+
+def group_for(sl, dims, nranks, u, recon=18):
+    g = sl.SlabGroup(dims, nranks, recon=recon)
+    g.load_gauge_from_global(torch.from_numpy(u))
+    return g
+
+
+def gathered(sl, parts):
+    return sl.gather_vector([p.cpu() for p in parts]).numpy()
+
+
+# lattice, number of slabs: T = 2 (every site on a slab boundary), ragged tiles, the 1-slab ring
+# (the periodic wrap itself goes through the mailbox), 16^4 in 2, 4, 8 slabs
+CASES = [((4, 4, 4, 4), 1), ((4, 4, 4, 4), 2), ((2, 2, 2, 4), 2), ((4, 2, 6, 8), 4), ((6, 4, 2, 12), 3),
+         ((10, 6, 6, 4), 2), ((8, 8, 8, 8), 2), ((8, 8, 8, 8), 4), ((16, 16, 16, 16), 2), ((16, 16, 16, 16), 8)]
+
+
+@pytest.mark.parametrize("recon", [18, 12])
+@pytest.mark.parametrize("dims,nranks", CASES)
+def test_slab_dslash_matches_global_oracle(sl, dims, nranks, recon):
+    seed = 4200 + sum(dims) + nranks
+    u = synth.gauge_field(dims, "haar", seed)
+    vh = synth.volume(dims) // 2
+    g = group_for(sl, dims, nranks, u, recon)
+    try:
+        for parity in (0, 1):
+            vin = synth.vector((3, vh), seed + 1 + parity)
+            want = oracle.dslash(dims, 0, u, parity, vin)
+            outs = g.dslash(parity, g.scatter(torch.from_numpy(vin)), g.new_vectors())
+            g.synchronize()
+            assert rel(gathered(sl, outs), want) <= DSLASH_TOL
+        # twice in a row with different inputs: the two ghost buffers alternate
+        for k in range(3):
+            vin = synth.vector((3, vh), seed + 10 + k)
+            outs = g.dslash(1, g.scatter(torch.from_numpy(vin)), g.new_vectors())
+            g.synchronize()
+            assert rel(gathered(sl, outs), oracle.dslash(dims, 0, u, 1, vin)) <= DSLASH_TOL
+    finally:
+        g.close()
+
+
+@pytest.mark.parametrize("dims,nranks", [((4, 4, 4, 4), 2), ((4, 2, 6, 8), 4), ((8, 8, 8, 8), 2), ((16, 16, 16, 16), 4)])
+def test_slab_MdagM_matches_global_oracle(sl, dims, nranks):
+    u = synth.gauge_field(dims, "smooth", 77 + nranks)
+    vin = synth.vector((3, synth.volume(dims) // 2), 78)
+    want = oracle.apply_MdagM(dims, 0, u, 0.07, vin)
+    g = group_for(sl, dims, nranks, u)
+    try:
+        outs = g.apply_MdagM(0.07, g.scatter(torch.from_numpy(vin)), g.new_vectors())
+        g.synchronize()
+        assert rel(gathered(sl, outs), want) <= DSLASH_TOL
+    finally:
+        g.close()
+
+
+def test_slab_boundary_sign_sits_on_the_global_boundary(sl):
+    """Unit links, constant vector: D v vanishes except on the two time-slices next to the GLOBAL
+    antiperiodic boundary, wherever the slabs are cut (reading A4)."""
+    dims, nranks = (4, 4, 4, 8), 4
+    v, vh, sh = synth.volume(dims), synth.volume(dims) // 2, 4 * 4 * 4 // 2
+    u = np.zeros((v, 4, 3, 3), complex)
+    u[:, :, [0, 1, 2], [0, 1, 2]] = 1.0
+    vin = np.ones((3, vh), complex)
+    g = group_for(sl, dims, nranks, u)
+    try:
+        outs = g.dslash(1, g.scatter(torch.from_numpy(vin)), g.new_vectors())
+        g.synchronize()
+        out = gathered(sl, outs).reshape(3, 8, sh)
+        assert np.abs(out[:, 1:7]).max() == 0.0
+        assert np.abs(np.abs(out[:, 0]) - 1.0).max() < 1e-15 and np.abs(np.abs(out[:, 7]) - 1.0).max() < 1e-15
+        assert rel(out.reshape(3, vh), oracle.dslash(dims, 0, u, 1, vin)) <= DSLASH_TOL
+    finally:
+        g.close()
+
+
+@pytest.mark.parametrize("recon", [18, 12])
+@pytest.mark.parametrize("cfg,nranks", [(1, 1), (1, 2), (2, 2), (2, 4), (2, 8)])
+def test_slab_cg_matches_global_oracle(sl, cfg, nranks, recon):
+    c, u, b = synth.config_inputs(cfg)
+    want = oracle.cg(c["dims"], 0, u, c["param"], c["tol"], 20000, b)
+    assert want["status"] == 0
+    g = group_for(sl, c["dims"], nranks, u, recon)
+    try:
+        xs, it, res, status = g.cg_solve(c["param"], c["tol"], 20000, g.scatter(torch.from_numpy(b)), g.new_vectors())
+        x = gathered(sl, xs)
+        assert status == 0
+        assert abs(it - want["iters"]) <= 2
+        assert rel(x, want["x"]) <= CG_TOL
+        assert res <= 2 * c["tol"]
+        # three synchronisation points per iteration, in step on every rank
+        assert len({s.sync_points() for s in g.slabs}) == 1
+    finally:
+        g.close()
+
+
+def test_slab_cg_fixed_iterations_and_rank_count_independence(sl):
+    """tol = 0: exactly k iterations.  The iterate agrees with the oracle's to rounding for every
+    number of slabs, and the batch size of the host loop does not change a bit of it."""
+    c, u, b = synth.config_inputs(2)
+    for k in (1, 6):
+        want = oracle.cg(c["dims"], 0, u, c["param"], 0.0, k, b)
+        for nranks in (1, 2, 8):
+            g = group_for(sl, c["dims"], nranks, u)
+            try:
+                ref = None
+                for every in (1, 5):
+                    g.set_option(sl.OPT_CHECK_EVERY, every)
+                    xs, it, res, status = g.cg_solve(c["param"], 0.0, k, g.scatter(torch.from_numpy(b)), g.new_vectors())
+                    x = gathered(sl, xs)
+                    assert status == 1 and it == k
+                    assert rel(x, want["x"]) <= 1e-12
+                    assert abs(res - want["true_residual"]) <= 1e-9 * want["true_residual"]
+                    if ref is None:
+                        ref = x
+                    assert np.array_equal(ref, x)
+            finally:
+                g.close()
+
+
+def test_slab_cg_agrees_with_the_single_gpu_solver(sl):
+    from paper_1311_2719_b200 import lqcd
+    c, u, b = synth.config_inputs(2)
+    with lqcd.Lattice(c["dims"], lqcd.STAGGERED) as lat:
+        lat.load_gauge(torch.from_numpy(u).cuda())
+        x1, it1, res1, st1 = lat.cg_solve(c["param"], c["tol"], 20000, torch.from_numpy(b).cuda())
+        x1 = x1.cpu().numpy()
+    g = group_for(sl, c["dims"], 4, u)
+    try:
+        xs, it, res, status = g.cg_solve(c["param"], c["tol"], 20000, g.scatter(torch.from_numpy(b)), g.new_vectors())
+        assert status == st1 == 0 and abs(it - it1) <= 2
+        assert rel(gathered(sl, xs), x1) <= CG_TOL
+    finally:
+        g.close()
+
+
+def test_slab_single_rank_entry_points(sl):
+    """lqcd_slab_dslash / _apply_MdagM / _cg_solve: the one-rank-per-process calls, here on the 1-slab
+    ring (its own neighbour on both sides), where signal and wait follow each other on one stream."""
+    c, u, b = synth.config_inputs(1)
+    dims = c["dims"]
+    s = sl.Slab(dims, 0, 1)
+    try:
+        s.connect([s.mailbox_ptr])
+        ug = torch.from_numpy(u)
+        s.load_gauge(sl.local_gauge(ug, dims, 0, 1).cuda(), sl.u3_below_from_global(ug, dims, 0, 1).cuda())
+        vin = synth.vector((3, synth.volume(dims) // 2), 5)
+        out = s.dslash(1, torch.from_numpy(vin).cuda(), s.new_vector())
+        s.stream.synchronize()
+        assert rel(out.cpu().numpy(), oracle.dslash(dims, 0, u, 1, vin)) <= DSLASH_TOL
+        out = s.apply_MdagM(0.1, torch.from_numpy(vin).cuda(), s.new_vector())
+        s.stream.synchronize()
+        assert rel(out.cpu().numpy(), oracle.apply_MdagM(dims, 0, u, 0.1, vin)) <= DSLASH_TOL
+        want = oracle.cg(dims, 0, u, c["param"], c["tol"], 20000, b)
+        x, it, res, status = s.cg_solve(c["param"], c["tol"], 20000, torch.from_numpy(b).cuda(), s.new_vector())
+        assert status == 0 and abs(it - want["iters"]) <= 2 and rel(x.cpu().numpy(), want["x"]) <= CG_TOL
+    finally:
+        s.close()
+
+
+def test_slab_edge_cases_and_errors(sl):
+    c, u, b = synth.config_inputs(1)
+    dims = c["dims"]
+    g = group_for(sl, dims, 2, u)
+    try:
+        zero = [torch.zeros_like(v) for v in g.scatter(torch.from_numpy(b))]
+        xs, it, res, status = g.cg_solve(0.1, 1e-10, 100, zero, g.new_vectors())          # b = 0 (reading A11)
+        assert it == 0 and res == 0.0 and status == 0 and not gathered(sl, xs).any()
+        xs, it, res, status = g.cg_solve(0.1, 1e-10, 0, g.scatter(torch.from_numpy(b)), g.new_vectors())
+        assert it == 0 and status == 1 and abs(res - 1.0) < 1e-15                          # no iteration: r = b
+        bs = g.scatter(torch.from_numpy(b))
+        with pytest.raises(sl.LqcdError):
+            g.cg_solve(0.1, 1e-10, 10, bs, bs)                                             # aliasing
+        with pytest.raises(sl.LqcdError):
+            g.dslash(2, bs, g.new_vectors())                                               # bad parity
+    finally:
+        g.close()
+    with pytest.raises(ValueError):
+        sl.SlabGroup((4, 4, 4, 4), 4)                                                      # T = 1
+    with pytest.raises(ValueError):
+        sl.SlabGroup((4, 4, 4, 6), 4)                                                      # 6 % 4
+    with pytest.raises(sl.LqcdError):
+        sl.Slab((4, 4, 4, 12), 0, 4)                                                       # T = 3 is odd
+    s = sl.Slab(dims, 0, 2)
+    try:
+        with pytest.raises(sl.LqcdError) as e:                                             # peers not connected
+            s.dslash(1, s.new_vector(), s.new_vector())
+        assert e.value.code == -3
+    finally:
+        s.close()
