@@ -149,6 +149,103 @@ def oracle_arm(cfg, u, b, steps, warmup, target_seconds=6.0):
                       % (n_it, cfg["name"], steps, sec), "ms_per_step": sec * 1e3, "iters_per_step": n_it}
 
 
+def slab_arm(args, cfg, workload, metric, ranks, device):
+    """--parallelism slab: ONE system on N GPUs, rank r owns time-slab r (strong scaling).  One process
+    per GPU; the mailboxes are mapped across processes with CUDA IPC; every hot step -- hopping terms,
+    halo stores into the neighbours' ghost faces, rank-ordered sums, the CG -- is in the CUDA library."""
+    import torch
+    from paper_1311_2719_b200 import slab as sl
+    if cfg["fermion"] != "staggered":
+        raise SystemExit("--parallelism slab is built for the staggered configs")
+    rank, world = ranks.rank, ranks.world
+    dims = cfg["dims"]
+    ug = torch.from_numpy(synth.gauge_field(dims, cfg["links"], cfg["seed"]))      # every rank builds the global field,
+    bg = torch.from_numpy(synth.source(dims, cfg["fermion"], cfg["seed"]))         # keeps its slab
+    s = sl.Slab(dims, rank, world, device=device)
+    s.set_option(sl.OPT_RECONSTRUCT, args.recon)
+    s.set_option(sl.OPT_CHECK_EVERY, args.check_every)
+    s.connect_ipc()
+    u_local = sl.local_gauge(ug, dims, rank, world).pin_memory()
+    u3_below = sl.u3_below_from_global(ug, dims, rank, world).pin_memory()
+    b_host = sl.local_vector(bg, dims, rank, world).pin_memory()
+    del ug, bg
+    s.load_gauge(u_local.to(device), u3_below.to(device))
+    b_dev, x_dev = b_host.to(device), s.new_vector()
+    maxiter = 100000
+    vh = synth.volume(dims) // 2
+    for _ in range(max(args.warmup, 3)):
+        _, iters, res, status = s.cg_solve(cfg["param"], cfg["tol"], maxiter, b_dev, x_dev)
+    assert status == 0, "CG did not converge"
+    sampler = ClockSampler(ranks.local_rank) if rank == 0 else None
+    launches0 = s.kernel_launches()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ranks.barrier()
+    e0.record(s.stream)
+    for _ in range(args.steps):
+        _, iters, res, status = s.cg_solve(cfg["param"], cfg["tol"], maxiter, b_dev, x_dev)
+    e1.record(s.stream)
+    ranks.barrier()
+    ms_solve = ranks.max(e0.elapsed_time(e1)) / args.steps
+    launches = ranks.sum(s.kernel_launches() - launches0)
+    value = cg_bytes(cfg, iters, args.recon) / (ms_solve * 1e-3) / 1e9            # the ONE global solve
+    # the slab hopping term alone (face push + synchronisation point + Dslash per call)
+    va, vb = s.new_vector(), s.new_vector()
+    va.copy_(b_dev)
+    for i in range(6):
+        s.dslash(1 - (i & 1), va if not (i & 1) else vb, vb if not (i & 1) else va)
+    d0, d1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ranks.barrier()
+    d0.record(s.stream)
+    for i in range(args.dslash_reps):
+        s.dslash(1 - (i & 1), va if not (i & 1) else vb, vb if not (i & 1) else va)
+    d1.record(s.stream)
+    ranks.barrier()
+    us_dslash = ranks.max(d0.elapsed_time(d1)) * 1e3 / args.dslash_reps
+    clocks = sampler.stop() if sampler else None
+    dbytes = STAG_DSLASH_BYTES - 8 * 8 * (18 - args.recon)
+    achieved = dbytes * vh / (us_dslash * 1e-6) / 1e9                              # all ranks together
+    peak, peak_src = hbm_peak()
+    # e2e: this rank's slab of u and b from pinned host memory, x back, inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        x_host = torch.empty(s.vector_shape, dtype=torch.complex128).pin_memory()
+        ranks.barrier()
+        t0 = time.perf_counter()
+        s.load_gauge(u_local.to(device, non_blocking=True), u3_below.to(device, non_blocking=True))
+        bd = b_host.to(device, non_blocking=True)
+        _, it_e, res_e, st_e = s.cg_solve(cfg["param"], cfg["tol"], maxiter, bd, x_dev)
+        x_host.copy_(x_dev)
+        torch.cuda.synchronize()
+        sec = ranks.max(time.perf_counter() - t0)
+        e2e = {"value": cg_bytes(cfg, it_e, args.recon) / sec / 1e9, "unit": "GB/s", "ms_per_step": sec * 1e3,
+               "h2d_bytes_per_step": int(ranks.sum((u_local.numel() + u3_below.numel() + b_host.numel()) * 16)),
+               "d2h_bytes_per_step": int(ranks.sum(x_host.numel() * 16 + 128)), "iters": it_e, "true_residual": res_e,
+               "api": "slab.Slab.load_gauge + cg_solve (pinned host u_local, b_local -> x_local)"}
+    if rank == 0:
+        line = {
+            "metric": metric, "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_solve, "higher_is_better": True, "scaling": "strong",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload, "precision": "f64", "reconstruct": args.recon, "cg_mode": "async",
+                       "check_every": args.check_every,
+                       "parallelism": "time-slabs x%d (one system; T = %d slices per GPU; peer-memory halo + sums)" % (world, dims[3] // world),
+                       "l2_policy": "inputs larger than L2 (%.0f MB of links per Dslash and GPU), no flush" % (2 * vh * 576 / 1e6 / world)},
+            "cg": {"time_to_solution_ms": ms_solve, "iters": iters, "true_residual": res,
+                   "us_per_iteration": ms_solve * 1e3 / max(iters, 1), "sync_points": s.sync_points()},
+            "dslash": {"us_per_call": us_dslash, "GBps": achieved, "GFLOPs": STAG_DSLASH_FLOPS * vh / (us_dslash * 1e-6) / 1e9,
+                       "reps": args.dslash_reps, "note": "lqcd_slab_dslash: face push + synchronisation point + hopping term"},
+            "roofline": {"bound": "hbm", "kernel": "stag_dslash_slab_kernel<SE_PLAIN> (+ face push, signal, wait)",
+                         "achieved": achieved / world, "peak": peak, "unit": "GB/s", "frac": achieved / world / peak,
+                         "peak_source": peak_src + "; achieved is per GPU", "traffic": None, "bytes_per_site": dbytes,
+                         "sites_per_launch": vh // world},
+            "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "cpu_baseline": None, "variants": None,
+        }
+        print(json.dumps(line))
+    s.close()
+    ranks.close()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -165,6 +262,10 @@ def main():
                     help="f64 = the fp64 conjugate gradient (the headline); mixed = fp32 iterations + fp64 reliable updates")
     ap.add_argument("--delta", type=float, default=0.1, help="reliable-update threshold of --precision mixed")
     ap.add_argument("--no-variants", action="store_true", help="skip the extra recon-12 / mixed-precision solves")
+    ap.add_argument("--parallelism", default="replicas", choices=["replicas", "slab"],
+                    help="N > 1: replicas = independent right-hand sides per GPU (weak scaling, the default); "
+                         "slab = ONE system cut into time-slabs, halo exchange and sums through peer memory "
+                         "(strong scaling; include/lqcd_slab.h; staggered configs)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -208,6 +309,9 @@ def main():
     device = torch.device("cuda", local_rank)
     ranks = Ranks(backend="nccl", device=device)
     barrier, max_over_ranks, sum_over_ranks = ranks.barrier, ranks.max, ranks.sum
+
+    if args.parallelism == "slab":
+        return slab_arm(args, cfg, workload, metric, ranks, device)
 
     f = lqcd.STAGGERED if cfg["fermion"] == "staggered" else lqcd.WILSON
     u = synth.gauge_field(cfg["dims"], cfg["links"], cfg["seed"])
@@ -271,13 +375,13 @@ def main():
         va.copy_(b_dev)
         vb.zero_()
         dbytes, dflops = WILSON_DSLASH_BYTES - 8 * 8 * (18 - args.recon), WILSON_DSLASH_FLOPS
-    for i in range(6):
-        lat.dslash(1 - (i & 1), va if not (i & 1) else vb, vb if not (i & 1) else va)
+    # lqcd_dslash_sweep enqueues the launches natively (odd parity first, ping-pong va -> vb -> va ...):
+    # no Python between launches, so the small lattices are timed on the device too.
+    lat.dslash_sweep(1, va, vb, 6)
     d0, d1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     d0.record(lat.stream)
-    for i in range(args.dslash_reps):
-        lat.dslash(1 - (i & 1), va if not (i & 1) else vb, vb if not (i & 1) else va)
+    lat.dslash_sweep(1, va, vb, args.dslash_reps)
     d1.record(lat.stream)
     barrier()
     us_dslash = max_over_ranks(d0.elapsed_time(d1)) * 1e3 / args.dslash_reps
@@ -331,6 +435,34 @@ def main():
                 "GBps": sum_over_ranks(cg_bytes(cfg, it_v, recon_v, nu_v)) / (ms_v * 1e-3) / 1e9}
         lat.set_option(lqcd.OPT_RECONSTRUCT, args.recon)
         lat.load_gauge(u_dev)
+        # The time-slab decomposition with all R slabs on THIS GPU, driven in
+        # lock-step on one stream: the kernels, peer stores and mailboxes of an R-GPU run, so the
+        # difference to the undivided solve is the cost of the decomposition itself (6 tiny kernels
+        # per iteration, smaller grids), not of any link.  One warm-up + one timed solve each.
+        if world == 1 and not mixed:
+            from paper_1311_2719_b200 import slab as slab_mod
+            ug, bg = torch.from_numpy(u), torch.from_numpy(b)
+            for R in (2, 4, 8):
+                if cfg["dims"][3] % R or (cfg["dims"][3] // R) % 2 or cfg["dims"][3] // R < 2:
+                    continue
+                grp = slab_mod.SlabGroup(cfg["dims"], R, recon=args.recon)
+                grp.set_option(slab_mod.OPT_CHECK_EVERY, args.check_every)
+                grp.load_gauge_from_global(ug)
+                bs, xs = grp.scatter(bg), grp.new_vectors()
+                g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                st = grp.slabs[0].stream
+                for rep in range(2):
+                    torch.cuda.synchronize()
+                    g0.record(st)
+                    _, it_g, res_g, st_g = grp.cg_solve(cfg["param"], cfg["tol"], maxiter, bs, xs)
+                    g1.record(st)
+                    torch.cuda.synchronize()
+                ms_g = g0.elapsed_time(g1)
+                variants["slab_group%d_on_one_gpu" % R] = {
+                    "time_to_solution_ms": ms_g, "iters": it_g, "true_residual": res_g, "converged": st_g == 0,
+                    "GBps": cg_bytes(cfg, it_g, args.recon) / (ms_g * 1e-3) / 1e9}
+                grp.close()
+                del grp, bs, xs
 
     # ---- the oracle beside it (rank 0, N = 1 only)
     cpu = None

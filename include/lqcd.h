@@ -120,6 +120,13 @@ int lqcd_get_tables(lqcd_ctx *ctx, int32_t *iup_host, int32_t *idn_host, int32_t
  * in_dev and out_dev must not alias. */
 int lqcd_dslash(lqcd_ctx *ctx, int out_parity, const double *in_dev, double *out_dev);
 
+/* Throughput sweep of the bare hopping term (BASELINE.json config 5 "Dslash throughput sweep"): `reps`
+ * back-to-back launches enqueued natively, ping-pong between the two vectors -- launch k computes
+ * parity (first_out_parity + k) mod 2 from the vector launch k-1 wrote (launch 0 reads a_dev and
+ * writes b_dev).  For timing only: no host round trip between launches, so lattices whose kernel
+ * is shorter than a ctypes call are still measured on the device.  Vectors as lqcd_dslash. */
+int lqcd_dslash_sweep(lqcd_ctx *ctx, int first_out_parity, double *a_dev, double *b_dev, int reps);
+
 /* out = A in.  Staggered: even-site vectors, A = mass^2 - D_eo D_oe.  Wilson: full-lattice
  * vectors, A = gamma5 M gamma5 M with M = 1 - kappa D_W.  No aliasing. */
 int lqcd_apply_MdagM(lqcd_ctx *ctx, double mass_or_kappa, const double *in_dev, double *out_dev);

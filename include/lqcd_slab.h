@@ -21,8 +21,9 @@
  * neighbour (sh*48 bytes per face).  The kernel that PRODUCES a vector stores its two boundary
  * slices straight into the neighbours' ghost faces through peer memory (NVLink); inner products
  * travel as one partial per rank into every rank's slot array and are added in rank order, so every
- * rank holds bit-identical scalars.  A synchronisation point is two tiny kernels (signal, bounded
- * wait + combine); nothing goes through the host.  All of that memory is the rank's MAILBOX.
+ * rank holds bit-identical scalars.  A synchronisation point (signal, bounded wait, combine) runs in
+ * the last block of the producing kernel when a rank drives its own slab, or as two tiny kernels in
+ * the *_group calls; nothing goes through the host.  All of that memory is the rank's MAILBOX.
  *
  * Collective semantics: every rank must make the same sequence of lqcd_slab_* compute calls with the
  * same scalar arguments.  A peer that never arrives makes the call fail with LQCD_ECOMM after the
@@ -55,7 +56,15 @@ enum { LQCD_SLAB_MAX_RANKS = 16 };
 enum {
     LQCD_SLAB_OPT_RECONSTRUCT = 0,  /* 18 or 12, as LQCD_OPT_RECONSTRUCT; invalidates the loaded links */
     LQCD_SLAB_OPT_CHECK_EVERY = 1,  /* iterations enqueued per convergence read-back, 1..1024 (default 8) */
-    LQCD_SLAB_OPT_TIMEOUT_MS = 2    /* wait timeout of a synchronisation point, 1..600000 (default 20000) */
+    LQCD_SLAB_OPT_TIMEOUT_MS = 2,   /* wait timeout of a synchronisation point, 1..600000 (default 20000) */
+    LQCD_SLAB_OPT_GRAPH = 3,        /* 1 (default): when every slab of the call runs on one stream, each batch of
+                                       CG iterations is replayed from one CUDA graph (an odd check_every is
+                                       rounded up to even); 0: kernel-by-kernel launches.  Same iterates. */
+    LQCD_SLAB_OPT_FUSE_SYNC = 4     /* one-rank-per-process calls only.  1 (default): the last block of every kernel
+                                       that ends in a sum (the Dslash kernels of the CG, the p-update, the init)
+                                       also signals, waits and combines, so an iteration is three launches and
+                                       the exchange costs no kernel boundary; 0: a separate small launch per
+                                       synchronisation point, as the *_group calls always do.  Same iterates. */
 };
 
 /* Slab of rank `rank` of `nranks` for the global L0 x L1 x L2 x L3 staggered lattice.  L3/nranks must be

@@ -718,6 +718,20 @@ int lqcd_dslash(lqcd_ctx* ctx, int out_parity, const double* in_dev, double* out
     return launch_wilson<WE_PLAIN, false>(ctx, wilson_args(ctx, out_parity, (const cplx*)in_dev, (cplx*)out_dev, 0.0));
 }
 
+int lqcd_dslash_sweep(lqcd_ctx* ctx, int first_out_parity, double* a_dev, double* b_dev, int reps)
+{
+    int rc = check_ready(ctx, true);
+    if (rc) return rc;
+    if (!a_dev || !b_dev || a_dev == b_dev) return fail(ctx, LQCD_EARG, "null or aliased vector pointer");
+    if (first_out_parity != LQCD_EVEN && first_out_parity != LQCD_ODD) return fail(ctx, LQCD_EARG, "bad parity %d", first_out_parity);
+    if (reps < 0) return fail(ctx, LQCD_EARG, "reps must be >= 0");
+    for (int k = 0; k < reps; ++k) {
+        rc = lqcd_dslash(ctx, (first_out_parity + k) & 1, (k & 1) ? b_dev : a_dev, (k & 1) ? a_dev : b_dev);
+        if (rc) return rc;
+    }
+    return LQCD_OK;
+}
+
 int lqcd_apply_MdagM(lqcd_ctx* ctx, double mass_or_kappa, const double* in_dev, double* out_dev)
 {
     int rc = check_ready(ctx, true);

@@ -41,7 +41,7 @@ struct lqcd_slab {
     cudaStream_t stream;
     int device;
     bool memory_set, connected, gauge_loaded;
-    int recon, check_every, timeout_ms;
+    int recon, check_every, timeout_ms, use_graph, fuse_sync;
     unsigned long long seq;  // synchronisation points passed
     CgScalars* h_sc;         // pinned, 2 slots
     SlabScalars* h_ss;       // pinned
@@ -205,6 +205,19 @@ int launch_stag(lqcd_slab* s, const StagArgsD& a)
     return LQCD_OK;
 }
 
+// The same kernel with the synchronisation point that follows it run by its last block.
+template <int EPI>
+int launch_stag_sync(lqcd_slab* s, const StagArgsD& a, const SlabSyncArgs& sy)
+{
+    const unsigned int grid = blocks_for(s->g.Vh, kStagBlock);
+    if (s->recon == 12)
+        stag_dslash_slab_sync_kernel<EPI, kStagBlock, 12, cplx><<<grid, kStagBlock, 0, s->stream>>>(a, sy);
+    else
+        stag_dslash_slab_sync_kernel<EPI, kStagBlock, 18, cplx><<<grid, kStagBlock, 0, s->stream>>>(a, sy);
+    SLAB_LAUNCH_CHECK();
+    return LQCD_OK;
+}
+
 int launch_push_faces(lqcd_slab* s, const cplx* v)
 {
     const unsigned int grid = blocks_for(6 * (size_t)s->sh, kVecBlock);
@@ -219,7 +232,6 @@ SlabSyncArgs sync_args(const lqcd_slab* s, int op, int nvals, double m2, double 
     memset(&a, 0, sizeof a);
     a.rank = s->rank;
     a.nranks = s->nranks;
-    a.seq = s->seq;
     a.nvals = nvals;
     a.own.flag = (unsigned long long*)(s->mb + s->mb_flag);
     a.own.slot = (double*)(s->mb + s->mb_slot);
@@ -241,9 +253,22 @@ SlabSyncArgs sync_args(const lqcd_slab* s, int op, int nvals, double m2, double 
 
 // One synchronisation point for the whole group: every slab signals, then every slab waits and
 // combines.  (With all slabs on one stream the signals therefore precede every wait: no kernel spins.)
-int group_sync(const Group& G, int op, int nvals, double m2 = 0.0, double tol = 0.0, int maxiter = 0)
+// A group of one -- a rank driving only its own slab -- does both in one launch.
+// in_producer: the producer kernel was launched with the synchronisation point in its last block
+// (fused(G)); only the host's count moves.
+int group_sync(const Group& G, int op, int nvals, double m2 = 0.0, double tol = 0.0, int maxiter = 0,
+               bool in_producer = false)
 {
-    for (int r = 0; r < G.n; ++r) G.s[r]->seq += 1;
+    for (int r = 0; r < G.n; ++r) G.s[r]->seq += 1;  // host copy: selects the ghost buffers; the kernels count on the device
+    if (in_producer) return LQCD_OK;
+    if (G.n == 1) {
+        lqcd_slab* s = G.s[0];
+        int rc = use_device(s);
+        if (rc) return rc;
+        slab_signal_wait_combine_kernel<<<1, 32, 0, s->stream>>>(sync_args(s, op, nvals, m2, tol, maxiter));
+        SLAB_LAUNCH_CHECK();
+        return LQCD_OK;
+    }
     for (int r = 0; r < G.n; ++r) {
         lqcd_slab* s = G.s[r];
         int rc = use_device(s);
@@ -260,6 +285,20 @@ int group_sync(const Group& G, int op, int nvals, double m2 = 0.0, double tol = 
     }
     return LQCD_OK;
 }
+
+struct GraphHolder {
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    ~GraphHolder()
+    {
+        if (exec) cudaGraphExecDestroy(exec);
+        if (graph) cudaGraphDestroy(graph);
+    }
+};
+
+// A rank that drives only its own slab runs each synchronisation point inside the producer kernel.
+// Never a group of several slabs: on one stream its producers would wait for kernels queued behind them.
+bool fused(const Group& G) { return G.n == 1 && G.s[0]->fuse_sync; }
 
 int ensure_host(lqcd_slab* s)
 {
@@ -358,15 +397,17 @@ int group_MdagM(const Group& G, double mass, const cplx* const* in, cplx* const*
 int group_iteration(const Group& G, double mass, cplx* const* x)
 {
     const double m2 = mass * mass;
+    const bool fz = fused(G);
     int rc;
     for (int r = 0; r < G.n; ++r) {  // S1: t = D_oe p, partial <t,t>; faces of t -> neighbours
         lqcd_slab* s = G.s[r];
         rc = use_device(s);
         if (rc) return rc;
-        rc = launch_stag<SE_NORM>(s, stag_args(s, LQCD_ODD, s->p(), s->t(), true));
+        const StagArgsD a = stag_args(s, LQCD_ODD, s->p(), s->t(), true);
+        rc = fz ? launch_stag_sync<SE_NORM>(s, a, sync_args(s, SLAB_OP_ALPHA, 1, m2, 0.0, 0)) : launch_stag<SE_NORM>(s, a);
         if (rc) return rc;
     }
-    rc = group_sync(G, SLAB_OP_ALPHA, 1, m2);  // S2
+    rc = group_sync(G, SLAB_OP_ALPHA, 1, m2, 0.0, 0, fz);  // S2
     if (rc) return rc;
     for (int r = 0; r < G.n; ++r) {  // S3: D_eo t fused with the x / r updates, partial <r,r>
         lqcd_slab* s = G.s[r];
@@ -377,20 +418,20 @@ int group_iteration(const Group& G, double mass, cplx* const* x)
         a.p = s->p();
         a.x = x[r];
         a.r = s->r();
-        rc = launch_stag<SE_CGUPDATE>(s, a);
+        rc = fz ? launch_stag_sync<SE_CGUPDATE>(s, a, sync_args(s, SLAB_OP_UPDATE, 1, 0.0, 0.0, 0)) : launch_stag<SE_CGUPDATE>(s, a);
         if (rc) return rc;
     }
-    rc = group_sync(G, SLAB_OP_UPDATE, 1);  // beta, exit test (S4 happens on every rank identically)
+    rc = group_sync(G, SLAB_OP_UPDATE, 1, 0.0, 0.0, 0, fz);  // beta, exit test (S4 happens on every rank identically)
     if (rc) return rc;
     for (int r = 0; r < G.n; ++r) {  // S5: p = r + beta p, partial <p,p>; faces of p -> neighbours
         lqcd_slab* s = G.s[r];
         rc = use_device(s);
         if (rc) return rc;
-        slab_cg_pupdate_kernel<kVecBlock><<<vec_grid(s), kVecBlock, 0, s->stream>>>(s->r(), s->p(), s->nvec, push_next(s),
-                                                                                   s->sc(), s->ss(), s->rs());
+        slab_cg_pupdate_kernel<kVecBlock><<<vec_grid(s), kVecBlock, 0, s->stream>>>(
+            s->r(), s->p(), s->nvec, push_next(s), s->sc(), s->ss(), s->rs(), sync_args(s, SLAB_OP_PP, 1, 0.0, 0.0, 0), fz ? 1 : 0);
         SLAB_LAUNCH_CHECK();
     }
-    return group_sync(G, SLAB_OP_PP, 1);
+    return group_sync(G, SLAB_OP_PP, 1, 0.0, 0.0, 0, fz);
 }
 
 int group_cg(const Group& G, double mass, double tol, int maxiter, const cplx* const* b, cplx* const* x, int* iters,
@@ -402,11 +443,12 @@ int group_cg(const Group& G, double mass, double tol, int maxiter, const cplx* c
         lqcd_slab* s = G.s[r];
         rc = use_device(s);
         if (rc) return rc;
-        slab_cg_init_kernel<kVecBlock><<<vec_grid(s), kVecBlock, 0, s->stream>>>(b[r], x[r], s->r(), s->p(), s->nvec,
-                                                                                push_next(s), s->ss(), s->rs());
+        slab_cg_init_kernel<kVecBlock><<<vec_grid(s), kVecBlock, 0, s->stream>>>(
+            b[r], x[r], s->r(), s->p(), s->nvec, push_next(s), s->ss(), s->rs(), sync_args(s, SLAB_OP_INIT, 1, 0.0, tol, maxiter),
+            fused(G) ? 1 : 0);
         SLAB_LAUNCH_CHECK();
     }
-    rc = group_sync(G, SLAB_OP_INIT, 1, 0.0, tol, maxiter);
+    rc = group_sync(G, SLAB_OP_INIT, 1, 0.0, tol, maxiter, fused(G));
     if (rc) return rc;
 
     // Host loop as LQCD_CG_ASYNC of lqcd_cg_solve: batches of check_every iterations are enqueued
@@ -414,16 +456,56 @@ int group_cg(const Group& G, double mass, double tol, int maxiter, const cplx* c
     // (signals and waits still run, so the ranks stay in step).  The scalars are bit-identical on all
     // ranks; rank 0's copy (of this process) is the one read.
     CgScalars* h = s0->h_sc;
-    const int batch = s0->check_every;
+    int batch = s0->check_every;
+    // With every slab on one stream (a rank alone, or the single-GPU group) the batch is captured once
+    // and replayed as a CUDA graph: the synchronisation kernels take their number from device memory,
+    // and an even count of synchronisation points per replay (3 per iteration, so an even batch)
+    // leaves the ghost-buffer parity baked into the captured kernels valid for every replay.
+    bool one_stream = s0->stream != nullptr;
+    for (int r = 1; r < G.n; ++r)
+        if (G.s[r]->stream != s0->stream || G.s[r]->device != s0->device) one_stream = false;
+    GraphHolder gh;
+    long long per_replay[LQCD_SLAB_MAX_RANKS] = { 0 };
+    if (s0->use_graph && one_stream && maxiter > 0) {
+        lqcd_slab* s = s0;
+        if (batch & 1) batch += 1;  // iterations after convergence are no-ops, so this changes nothing
+        unsigned long long seq0[LQCD_SLAB_MAX_RANKS];
+        long long launched0[LQCD_SLAB_MAX_RANKS];
+        for (int r = 0; r < G.n; ++r) {
+            seq0[r] = G.s[r]->seq;
+            launched0[r] = G.s[r]->launches;
+        }
+        SLAB_CUDA(cudaStreamBeginCapture(s0->stream, cudaStreamCaptureModeThreadLocal));
+        rc = LQCD_OK;
+        for (int k = 0; k < batch && !rc; ++k) rc = group_iteration(G, mass, x);
+        cudaError_t ce = cudaStreamEndCapture(s0->stream, &gh.graph);
+        for (int r = 0; r < G.n; ++r) {  // capturing ran nothing
+            per_replay[r] = G.s[r]->launches - launched0[r];
+            G.s[r]->launches = launched0[r];
+            G.s[r]->seq = seq0[r];
+        }
+        if (rc) return rc;
+        SLAB_CUDA(ce);
+        SLAB_CUDA(cudaGraphInstantiate(&gh.exec, gh.graph, 0));
+    }
     int slot = 0;
     bool pending[2] = { false, false };
     bool finished = false;
     long long enqueued = 0;
     while (!finished) {
         if (enqueued < (long long)maxiter) {
-            for (int k = 0; k < batch; ++k) {
-                rc = group_iteration(G, mass, x);
-                if (rc) return rc;
+            if (gh.exec) {
+                lqcd_slab* s = s0;
+                SLAB_CUDA(cudaGraphLaunch(gh.exec, s0->stream));
+                for (int r = 0; r < G.n; ++r) {
+                    G.s[r]->seq += 3ull * (unsigned long long)batch;
+                    G.s[r]->launches += per_replay[r];
+                }
+            } else {
+                for (int k = 0; k < batch; ++k) {
+                    rc = group_iteration(G, mass, x);
+                    if (rc) return rc;
+                }
             }
             enqueued += batch;
         }
@@ -455,10 +537,10 @@ int group_cg(const Group& G, double mass, double tol, int maxiter, const cplx* c
         a.m2 = mass * mass;
         a.p = x[r];
         a.b = b[r];
-        rc = launch_stag<SE_RESIDUAL>(s, a);
+        rc = fused(G) ? launch_stag_sync<SE_RESIDUAL>(s, a, sync_args(s, SLAB_OP_RES2, 1, 0.0, 0.0, 0)) : launch_stag<SE_RESIDUAL>(s, a);
         if (rc) return rc;
     }
-    rc = group_sync(G, SLAB_OP_RES2, 1);
+    rc = group_sync(G, SLAB_OP_RES2, 1, 0.0, 0.0, 0, fused(G));
     if (rc) return rc;
     rc = use_device(s0);
     if (rc) return rc;
@@ -511,6 +593,8 @@ int lqcd_slab_create(lqcd_slab** out, int L0, int L1, int L2, int L3, int rank, 
     c->recon = 18;
     c->check_every = 8;
     c->timeout_ms = 20000;
+    c->use_graph = 1;
+    c->fuse_sync = 1;
 
     size_t off = 0;
     const size_t vec_bytes = align_up(c->nvec * sizeof(cplx));
@@ -615,6 +699,16 @@ int lqcd_slab_set_option(lqcd_slab* s, int option, int value)
     if (option == LQCD_SLAB_OPT_TIMEOUT_MS) {
         if (value < 1 || value > 600000) return fail(s, LQCD_EARG, "timeout must be in 1..600000 ms");
         s->timeout_ms = value;
+        return LQCD_OK;
+    }
+    if (option == LQCD_SLAB_OPT_FUSE_SYNC) {
+        if (value != 0 && value != 1) return fail(s, LQCD_EARG, "fuse_sync must be 0 or 1");
+        s->fuse_sync = value;
+        return LQCD_OK;
+    }
+    if (option == LQCD_SLAB_OPT_GRAPH) {
+        if (value != 0 && value != 1) return fail(s, LQCD_EARG, "graph must be 0 or 1");
+        s->use_graph = value;
         return LQCD_OK;
     }
     return fail(s, LQCD_EARG, "unknown option %d", option);

@@ -143,6 +143,41 @@ __device__ __forceinline__ void grid_sum(double local, const ReduceScratch& rs, 
     }
 }
 
+// As grid_sum, but `fin(total)` is called by EVERY thread of the last block (total broadcast): for
+// finalisers that talk to other GPUs (slab_sync_tail).  `wrote_peer`: this thread stored into another
+// GPU's memory; a block in which any thread did fences at SYSTEM scope before it takes the ticket
+// (membar.sys in every block costs ~20 us on a 4096-block kernel, so only those blocks pay it).
+template <int BLOCK, class Finalise>
+__device__ __forceinline__ void grid_sum_block(double local, bool wrote_peer, const ReduceScratch& rs, Finalise fin)
+{
+    __shared__ bool is_last_b;
+    __shared__ double total_b;
+    const int any_peer = __syncthreads_or(wrote_peer ? 1 : 0);
+    double s = block_sum<BLOCK>(local);
+    if (threadIdx.x == 0) {
+        rs.partials[blockIdx.x] = s;
+        if (any_peer)
+            __threadfence_system();
+        else
+            __threadfence();
+        unsigned int t = atomicAdd(rs.ticket, 1u);
+        is_last_b = (t == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (is_last_b) {
+        __threadfence();
+        double acc = 0.0;
+        for (unsigned int i = threadIdx.x; i < gridDim.x; i += BLOCK) acc += __ldcg(rs.partials + i);
+        double total = block_sum<BLOCK>(acc);
+        if (threadIdx.x == 0) {
+            *rs.ticket = 0u;
+            total_b = total;
+        }
+        __syncthreads();
+        fin(total_b);
+    }
+}
+
 // The same for N sums at once (partials laid out [N][gridDim.x]); `fin(total[N])`.
 template <int BLOCK, int N, class Finalise>
 __device__ __forceinline__ void grid_sum_n(const double (&local)[N], const ReduceScratch& rs, Finalise fin)

@@ -15,6 +15,7 @@
 // = 1248 B, the figure the roofline is quoted on.
 #pragma once
 #include "reduce.cuh"
+#include "slab_sync.cuh"
 
 namespace lqcd {
 
@@ -79,30 +80,25 @@ __device__ __forceinline__ void stag_hop(const StagArgs<C>& a, const Site& s, C 
     C U[9], W[9], vf[3], vb[3];
     double sf, sb;
     if (SLAB && MU == 3) {
-        // time hops of a slab: no wrap inside the slab; the two boundary slices read the ghost faces
-        // (written by the neighbour ranks through peer memory: L2 loads, never the read-only path)
+        // Time hops of a slab: no wrap inside the slab; the two boundary slices read the ghost faces the
+        // neighbour ranks stored through peer memory.  One code path: base pointer and colour stride are
+        // selected, then the loads are those of the undivided kernel.  L2 loads (ld.cg) throughout --
+        // never the read-only path for peer-written data; the t+-1 neighbours are sh sites away, in
+        // other blocks, so L1 would not have helped.
         const bool top = s.x3 + 1 == a.g.L3, bottom = s.x3 == 0;
         const size_t sh = (size_t)a.sl.sh;
+        const C* vfp = top ? a.sl.ghost_hi + (s.e - (a.g.L3 - 1) * a.g.s3) : a.in + (s.e + a.g.s3);
+        const size_t vfs = top ? sh : Vh;
+        const C* vbp = bottom ? a.sl.ghost_lo + s.e : a.in + (s.e - a.g.s3);
+        const C* Ub = bottom ? a.sl.gauge_ghost + (size_t)((1 - a.parity) * NC) * sh + s.e
+                             : a.gauge + (size_t)(((1 - a.parity) * 4 + MU) * NC) * Vh + (s.e - a.g.s3);
+        const size_t vbs = bottom ? sh : Vh;
         load_link<RECON>(Uf, Vh, U);
-        if (top) {
-            const C* v = a.sl.ghost_hi + (s.e - (a.g.L3 - 1) * a.g.s3);
 #pragma unroll
-            for (int c = 0; c < 3; ++c) vf[c] = __ldcg(v + c * sh);
-        } else {
+        for (int c = 0; c < 3; ++c) vf[c] = __ldcg(vfp + c * vfs);
+        load_link<RECON>(Ub, vbs, W);
 #pragma unroll
-            for (int c = 0; c < 3; ++c) vf[c] = ld_keep(a.in + c * Vh + s.e + a.g.s3);
-        }
-        if (bottom) {
-            load_link<RECON>(a.sl.gauge_ghost + (size_t)((1 - a.parity) * NC) * sh + s.e, sh, W);
-            const C* v = a.sl.ghost_lo + s.e;
-#pragma unroll
-            for (int c = 0; c < 3; ++c) vb[c] = __ldcg(v + c * sh);
-        } else {
-            const int eb = s.e - a.g.s3;
-            load_link<RECON>(a.gauge + (size_t)(((1 - a.parity) * 4 + MU) * NC) * Vh + eb, Vh, W);
-#pragma unroll
-            for (int c = 0; c < 3; ++c) vb[c] = ld_keep(a.in + c * Vh + eb);
-        }
+        for (int c = 0; c < 3; ++c) vb[c] = __ldcg(vbp + c * vbs);
         // antiperiodic boundary of the GLOBAL lattice (reading A4)
         sf = (a.sl.t0 + s.x3 + 1 == a.sl.L3g) ? -eta : eta;
         sb = (a.sl.t0 + s.x3 == 0) ? eta : -eta;
@@ -180,8 +176,10 @@ __device__ __forceinline__ void slab_push(const StagArgs<C>& a, int x3, int e, c
     }
 }
 
+// `sy` (slab kernels only): non-null = this kernel's LAST block also runs the synchronisation point
+// that follows it (slab_sync_tail); null = the host launches the synchronisation kernels.
 template <int EPI, int BLOCK, int RECON, bool SLAB, class C>
-__device__ __forceinline__ void stag_dslash_body(const StagArgs<C>& a)
+__device__ __forceinline__ void stag_dslash_body(const StagArgs<C>& a, const SlabSyncArgs* sy = nullptr)
 {
     if (EPI == SE_NORM || EPI == SE_CGUPDATE || EPI == SE_CGUPDATE_MIXED) {
         // converged earlier, or waiting for a reliable update: this (pre-enqueued) iteration is a no-op
@@ -200,8 +198,12 @@ __device__ __forceinline__ void stag_dslash_body(const StagArgs<C>& a)
         stag_hop<2, RECON, SLAB>(a, s, acc);
         stag_hop<3, RECON, SLAB>(a, s, acc);
     }
+    bool wrote_peer = false;
     if (SLAB && (EPI == SE_PLAIN || EPI == SE_NORM)) {
-        if (active) slab_push(a, x3, e, acc);
+        if (active) {
+            slab_push(a, x3, e, acc);
+            wrote_peer = a.sl.push_lo != nullptr && (x3 == 0 || x3 + 1 == a.g.L3);
+        }
     }
     if (SLAB && EPI != SE_PLAIN && EPI != SE_MDAGM) {
         // Slab epilogues with a sum: the same per-site arithmetic as below, but the total over this
@@ -242,8 +244,12 @@ __device__ __forceinline__ void stag_dslash_body(const StagArgs<C>& a)
                 }
             }
         }
-        double* part = a.sl.part;
-        grid_sum<BLOCK>(local, a.rs, [part](double v) { part[0] = v; });
+        if (sy != nullptr) {
+            grid_sum_block<BLOCK>(local, wrote_peer, a.rs, [sy](double v) { slab_sync_tail<BLOCK>(*sy, v); });
+        } else {
+            double* part = a.sl.part;
+            grid_sum<BLOCK>(local, a.rs, [part](double v) { part[0] = v; });
+        }
         return;
     }
     if (EPI == SE_PLAIN) {
@@ -372,6 +378,14 @@ template <int EPI, int BLOCK, int RECON, class C>
 __global__ void __launch_bounds__(BLOCK, StagMinBlocks<RECON, C>::value) stag_dslash_slab_kernel(const StagArgs<C> a)
 {
     stag_dslash_body<EPI, BLOCK, RECON, true>(a);
+}
+
+// ... with the synchronisation point that follows it run by its last block (one rank per process).
+template <int EPI, int BLOCK, int RECON, class C>
+__global__ void __launch_bounds__(BLOCK, StagMinBlocks<RECON, C>::value)
+stag_dslash_slab_sync_kernel(const StagArgs<C> a, const SlabSyncArgs sy)
+{
+    stag_dslash_body<EPI, BLOCK, RECON, true>(a, &sy);
 }
 
 }  // namespace lqcd

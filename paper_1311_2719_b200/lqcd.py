@@ -66,6 +66,7 @@ def load_library():
     L.lqcd_load_gauge.argtypes = [P, P]
     L.lqcd_get_tables.argtypes = [P, P, P, P]
     L.lqcd_dslash.argtypes = [P, I, P, P]
+    L.lqcd_dslash_sweep.argtypes = [P, I, P, P, I]
     L.lqcd_apply_MdagM.argtypes = [P, D, P, P]
     L.lqcd_cg_solve.argtypes = [P, D, D, I, P, P, ctypes.POINTER(I), ctypes.POINTER(D)]
     L.lqcd_cg_solve_mixed.argtypes = [P, D, D, I, D, P, P, ctypes.POINTER(I), ctypes.POINTER(I), ctypes.POINTER(D)]
@@ -204,6 +205,13 @@ class Lattice:
         self._check(self._lib.lqcd_dslash(self._ctx, int(out_parity), _cptr(vin), _cptr(out)))
         self._sync_out()
         return out
+
+    def dslash_sweep(self, first_out_parity: int, a: torch.Tensor, b: torch.Tensor, reps: int) -> None:
+        """`reps` back-to-back hopping terms enqueued natively, ping-pong a -> b -> a ... (timing only)."""
+        self._vec(a, "a")
+        self._vec(b, "b")
+        self._sync_in()
+        self._check(self._lib.lqcd_dslash_sweep(self._ctx, int(first_out_parity), _cptr(a), _cptr(b), int(reps)))
 
     def apply_MdagM(self, mass_or_kappa: float, vin: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:
         self._vec(vin, "in")

@@ -148,6 +148,26 @@ def test_slab_cg_fixed_iterations_and_rank_count_independence(sl):
                 g.close()
 
 
+@pytest.mark.parametrize("nranks", [1, 4])
+def test_slab_cg_graph_replay_changes_no_bit(sl, nranks):
+    """LQCD_SLAB_OPT_GRAPH: the batch of iterations replayed from a CUDA graph (synchronisation numbers
+    counted on the device, ghost buffers alternating inside the graph) against kernel-by-kernel launches."""
+    c, u, b = synth.config_inputs(2)
+    g = group_for(sl, c["dims"], nranks, u)
+    try:
+        got = []
+        for graph, every in ((0, 4), (1, 4), (1, 3), (1, 16)):
+            g.set_option(sl.OPT_GRAPH, graph)
+            g.set_option(sl.OPT_CHECK_EVERY, every)
+            xs, it, res, status = g.cg_solve(c["param"], c["tol"], 20000, g.scatter(torch.from_numpy(b)), g.new_vectors())
+            got.append((gathered(sl, xs), it, res, status))
+        for x, it, res, status in got[1:]:
+            assert status == 0 and it == got[0][1] and res == got[0][2] and np.array_equal(x, got[0][0])
+        assert len({s.sync_points() for s in g.slabs}) == 1
+    finally:
+        g.close()
+
+
 def test_slab_cg_agrees_with_the_single_gpu_solver(sl):
     from paper_1311_2719_b200 import lqcd
     c, u, b = synth.config_inputs(2)
@@ -186,6 +206,37 @@ def test_slab_single_rank_entry_points(sl):
         assert status == 0 and abs(it - want["iters"]) <= 2 and rel(x.cpu().numpy(), want["x"]) <= CG_TOL
     finally:
         s.close()
+
+
+def test_slab_fused_synchronisation_changes_no_bit(sl):
+    """One rank per process: the synchronisation point inside the last block of the producer kernels
+    (LQCD_SLAB_OPT_FUSE_SYNC, default) against separate launches, with and without graph replay, and
+    against the group call on the same 1-slab ring."""
+    c, u, b = synth.config_inputs(2)
+    dims = c["dims"]
+    ug = torch.from_numpy(u)
+    s = sl.Slab(dims, 0, 1)
+    g = group_for(sl, dims, 1, u)
+    try:
+        s.connect([s.mailbox_ptr])
+        s.load_gauge(sl.local_gauge(ug, dims, 0, 1).cuda(), sl.u3_below_from_global(ug, dims, 0, 1).cuda())
+        got = []
+        for fuse, graph in ((1, 1), (1, 0), (0, 1), (0, 0)):
+            s.set_option(sl.OPT_FUSE_SYNC, fuse)
+            s.set_option(sl.OPT_GRAPH, graph)
+            before = s.kernel_launches()
+            x, it, res, status = s.cg_solve(c["param"], c["tol"], 20000, torch.from_numpy(b).cuda(), s.new_vector())
+            got.append((x.cpu().numpy(), it, res, status, s.kernel_launches() - before))
+        xs, it, res, status = g.cg_solve(c["param"], c["tol"], 20000, g.scatter(torch.from_numpy(b)), g.new_vectors())
+        got.append((gathered(sl, xs), it, res, status, 0))
+        for x, it, res, status, _ in got[1:]:
+            assert status == 0 and it == got[0][1] and res == got[0][2] and np.array_equal(x, got[0][0])
+        assert got[0][4] < got[2][4]            # fused: three launches per iteration instead of six
+        want = oracle.cg(dims, 0, u, c["param"], c["tol"], 20000, b)
+        assert abs(got[0][1] - want["iters"]) <= 2 and rel(got[0][0], want["x"]) <= CG_TOL
+    finally:
+        s.close()
+        g.close()
 
 
 def test_slab_edge_cases_and_errors(sl):
