@@ -85,7 +85,12 @@ enum {
     LQCD_OPT_RECONSTRUCT = 2,
     /* 64 (default): lqcd_congrad_host solves with lqcd_cg_solve.  32: with lqcd_cg_solve_mixed
      * (delta = 0.1; staggered contexts only). */
-    LQCD_OPT_CONGRAD_PRECISION = 3
+    LQCD_OPT_CONGRAD_PRECISION = 3,
+    /* 1 (default): the fp32 kernels of lqcd_cg_solve_mixed give each thread two neighbouring sites and
+     * read them with 128-bit loads (lattices with L0 % 4 == 0; others use the one-site kernels).
+     * 0: one site per thread.  The vectors are bit-identical either way; the partial sums are
+     * grouped differently, so scalars differ in the last bits. */
+    LQCD_OPT_F32_PAIRS = 4
 };
 
 /* Create a context for an L0 x L1 x L2 x L3 lattice (every extent even and >= 2; L = 2 is

@@ -12,6 +12,7 @@
 #include "../../include/lqcd.h"
 #include "cg_kernels.cuh"
 #include "stag_dslash.cuh"
+#include "stag_dslash_f32x2.cuh"
 #include "wilson_dslash.cuh"
 
 using namespace lqcd;
@@ -52,6 +53,7 @@ struct lqcd_ctx {
     int check_every;
     int recon;  // 18 or 12 stored reals per link
     int congrad_precision;  // 64 or 32: which solver lqcd_congrad_host runs
+    int f32_pairs;          // fp32 kernels of the mixed solver: two sites per thread with 128-bit loads
     bool wilson_eo;  // set while lqcd_wilson_solve_eo runs: the CG works on Mhat^+ Mhat, even half of the vectors
     // host side
     CgScalars* h_sc;  // pinned, 2 slots
@@ -190,6 +192,15 @@ StagArgsF stag_args_f(const lqcd_ctx* ctx, int parity, const cplxf* in, cplxf* o
 template <int EPI>
 int launch_stag_f(lqcd_ctx* ctx, const StagArgsF& a)
 {
+    if (ctx->f32_pairs && ctx->g.Lh % 2 == 0) {  // two sites per thread, 128-bit loads (stag_dslash_f32x2.cuh)
+        const unsigned int grid2 = blocks_for((size_t)ctx->g.Vh / 2, kStagBlock);
+        if (ctx->recon == 12)
+            stag_dslash_f32x2_kernel<EPI, kStagBlock, 12><<<grid2, kStagBlock, 0, ctx->stream>>>(a);
+        else
+            stag_dslash_f32x2_kernel<EPI, kStagBlock, 18><<<grid2, kStagBlock, 0, ctx->stream>>>(a);
+        LQCD_LAUNCH_CHECK();
+        return LQCD_OK;
+    }
     const unsigned int grid = blocks_for(ctx->g.Vh, kStagBlock);
     if (ctx->recon == 12)
         stag_dslash_kernel<EPI, kStagBlock, 12, cplxf><<<grid, kStagBlock, 0, ctx->stream>>>(a);
@@ -437,6 +448,12 @@ int mixed_iteration_kernels(lqcd_ctx* ctx, double mass)  // S1 + S2, S3 on the f
 
 int mixed_pupdate(lqcd_ctx* ctx)  // S5 on the fp32 copies
 {
+    if (ctx->f32_pairs && ctx->nvec % 2 == 0) {
+        cg_pupdate_f32x2_kernel<kVecBlock><<<vec_grid(ctx), kVecBlock, 0, ctx->stream>>>(ctx->rf(), ctx->pf(), ctx->nvec, ctx->sc(),
+                                                                                       ctx->rs());
+        LQCD_LAUNCH_CHECK();
+        return LQCD_OK;
+    }
     cg_pupdate_kernel<kVecBlock, cplxf><<<vec_grid(ctx), kVecBlock, 0, ctx->stream>>>(ctx->rf(), ctx->pf(), vec_layout(ctx),
                                                                                       ctx->sc(), ctx->rs());
     LQCD_LAUNCH_CHECK();
@@ -577,6 +594,7 @@ int lqcd_create(lqcd_ctx** out, int L0, int L1, int L2, int L3, int fermion_type
     c->check_every = 4;
     c->recon = 18;
     c->congrad_precision = 64;
+    c->f32_pairs = 1;
 
     size_t off = 0;
     const size_t vec_bytes = align_up(c->nvec * sizeof(cplx));
@@ -666,6 +684,11 @@ int lqcd_set_option(lqcd_ctx* ctx, int option, int value)
         if (value != 64 && !(value == 32 && ctx->fermion == LQCD_STAGGERED))
             return fail(ctx, LQCD_EARG, "congrad precision must be 64, or 32 on a staggered context");
         ctx->congrad_precision = value;
+        return LQCD_OK;
+    }
+    if (option == LQCD_OPT_F32_PAIRS) {
+        if (value != 0 && value != 1) return fail(ctx, LQCD_EARG, "f32_pairs must be 0 or 1");
+        ctx->f32_pairs = value;
         return LQCD_OK;
     }
     return fail(ctx, LQCD_EARG, "unknown option %d", option);

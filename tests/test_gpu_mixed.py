@@ -93,6 +93,34 @@ def test_mixed_cg_modes_and_batching_give_identical_results(lq):
         assert status == 0 and abs(it - want["iters"]) <= 2 and rel(x.cpu().numpy(), want["x"]) <= 1e-9
 
 
+@pytest.mark.parametrize("recon", [18, 12])
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (8, 4, 6, 2), (12, 2, 2, 4), (4, 6, 10, 8), (16, 16, 16, 16)])
+def test_mixed_cg_two_sites_per_thread_kernels(lq, dims, recon):
+    """LQCD_OPT_F32_PAIRS (default on where L0 % 4 == 0): two sites per thread with 128-bit loads.  Same
+    per-site arithmetic as the one-site kernels -- only the partial sums are grouped differently, so
+    fixed-iteration iterates agree far below fp32 accuracy -- and the same parity with the oracle."""
+    mass = 0.08
+    u = synth.gauge_field(dims, "haar", 211)
+    b = synth.source(dims, "staggered", 212)
+    with lattice(lq, dims, u, recon) as lat:
+        for k in (1, 7):
+            got = []
+            for pairs in (1, 0):
+                lat.set_option(lq.OPT_F32_PAIRS, pairs)
+                x, it, nupd, res, status = lat.cg_solve_mixed(mass, 0.0, k, dev(b))
+                got.append((x.cpu().numpy(), it, lat.cg_history().numpy()))
+            assert got[0][1] == got[1][1] == k
+            assert rel(got[0][0], got[1][0]) <= 1e-6
+            assert np.allclose(got[0][2], got[1][2], rtol=1e-6)
+            want = oracle.cg_mixed(dims, u, mass, 0.0, k, b)
+            assert rel(got[0][0], want["x"]) <= 2e-5
+        lat.set_option(lq.OPT_F32_PAIRS, 1)
+        want = oracle.cg_mixed(dims, u, mass, 1e-10, 20000, b)
+        x, it, nupd, res, status = lat.cg_solve_mixed(mass, 1e-10, 20000, dev(b))
+        assert status == 0 and res <= 1e-10 and count_close(it, want["iters"]) and abs(nupd - want["updates"]) <= 2
+        assert np.linalg.norm(x.cpu().numpy() - want["x"]) <= 1e-8 * np.linalg.norm(want["x"])
+
+
 def test_mixed_cg_fixed_iterations_and_edge_cases(lq):
     dims, mass = (8, 8, 8, 4), 0.1
     u = synth.gauge_field(dims, "haar", 113)

@@ -269,3 +269,67 @@ def test_slab_edge_cases_and_errors(sl):
         assert e.value.code == -3
     finally:
         s.close()
+
+
+# ------------------------------------------------------------------ CUDA IPC plumbing, two processes on the one GPU
+def _ipc_worker(rank, world, port, out):
+    """Maps the peer's mailbox through lqcd_slab_ipc_export / _open and moves bytes with plain copies.
+    No compute call is made: kernels of two processes that wait for each other must not share a GPU."""
+    import ctypes
+    import os
+    import sys
+    os.environ.update(RANK=str(rank), LOCAL_RANK="0", WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+    import torch
+    import torch.distributed as dist
+    from paper_1311_2719_b200 import slab as sl
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    ok, msg = False, ""
+    try:
+        dims = (8, 8, 8, 8)
+        s = sl.Slab(dims, rank, world, device="cuda:0")
+        s.connect_ipc()                                     # all-gather of the handles over gloo, open, connect, barrier
+        lib = s._lib
+        # the peer's mailbox as this process sees it: write a pattern at a rank-dependent offset of its ghost area
+        nbytes = lib.lqcd_slab_mailbox_bytes(s._s)
+        other = 1 - rank
+        peer_ptr = s._opened[0][0]
+        pattern = torch.full((1024,), 100.0 + rank, dtype=torch.float64, device="cuda:0")
+        off = nbytes - 2 * 8192 + rank * 8192              # the tail of the ghost faces: unused by anything else here
+        try:
+            rt = ctypes.CDLL("libcudart.so.12")            # the runtime torch has already loaded
+        except OSError:
+            rt = ctypes.CDLL("/usr/local/cuda/lib64/libcudart.so.12")
+        rt.cudaMemcpy.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int]
+        rc = rt.cudaMemcpy(ctypes.c_void_p(peer_ptr + off), ctypes.c_void_p(pattern.data_ptr()), 8192, 3)
+        torch.cuda.synchronize()
+        dist.barrier()
+        # what the peer wrote into MY mailbox
+        mine = torch.empty(1024, dtype=torch.float64, device="cuda:0")
+        rc2 = rt.cudaMemcpy(ctypes.c_void_p(mine.data_ptr()), ctypes.c_void_p(s.mailbox_ptr + nbytes - 2 * 8192 + other * 8192), 8192, 3)
+        torch.cuda.synchronize()
+        ok = rc == 0 and rc2 == 0 and bool((mine == 100.0 + other).all().item())
+        dist.barrier()
+        s.close()
+    except Exception as e:  # pragma: no cover - reported through the queue
+        msg = repr(e)
+    out.put(dict(rank=rank, ok=ok, msg=msg))
+    dist.destroy_process_group()
+
+
+def test_slab_ipc_mailboxes_between_two_processes():
+    import socket
+    import torch.multiprocessing as mp
+    sock = socket.socket()
+    sock.bind(("127.0.0.1", 0))
+    port = sock.getsockname()[1]
+    sock.close()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_ipc_worker, args=(i, 2, port, q)) for i in range(2)]
+    for p in procs:
+        p.start()
+    got = sorted((q.get(timeout=300) for _ in procs), key=lambda d: d["rank"])
+    for p in procs:
+        p.join(timeout=120)
+    assert all(g["ok"] for g in got), got
