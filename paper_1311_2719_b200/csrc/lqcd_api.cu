@@ -20,7 +20,10 @@ using namespace lqcd;
 namespace {
 
 constexpr int kStagBlock = 128;
-constexpr int kWilsonBlock = 128;
+#ifndef LQCD_WILSON_BLOCK
+#define LQCD_WILSON_BLOCK 128
+#endif
+constexpr int kWilsonBlock = LQCD_WILSON_BLOCK;
 constexpr int kVecBlock = 256;
 constexpr int kReorderTile = 64;
 constexpr size_t kAlign = 256;

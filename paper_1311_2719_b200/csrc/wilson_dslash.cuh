@@ -15,6 +15,13 @@
 #pragma once
 #include "reduce.cuh"
 
+// Minimum resident blocks per SM.  Left alone ptxas takes 132-148 registers (3 blocks of 128 threads per
+// SM); capped at 128 registers a fourth block fits and the CG on 16^3 x 32 runs 16 % faster (sweep on
+// B200, cfg 4, us per iteration at 1..6 blocks: 145.2 145.0 146.0 122.2 141.7 160.5; profiles/r01_bench.md).
+#ifndef LQCD_WILSON_MINB
+#define LQCD_WILSON_MINB 4
+#endif
+
 namespace lqcd {
 
 enum WilsonEpilogue {
@@ -120,7 +127,7 @@ __device__ __forceinline__ void wilson_dir(const WilsonArgs& a, const Site& s, i
 }
 
 template <int EPI, bool DAGGER, int BLOCK, int RECON>
-__global__ void __launch_bounds__(BLOCK) wilson_dslash_kernel(const WilsonArgs a)
+__global__ void __launch_bounds__(BLOCK, LQCD_WILSON_MINB) wilson_dslash_kernel(const WilsonArgs a)
 {
     if (EPI == WE_M_NORM || EPI == WE_CGUPDATE || EPI == WE_EO_XPAY_NORM || EPI == WE_EO_CGUPDATE) {
         if (a.sc->done) return;
