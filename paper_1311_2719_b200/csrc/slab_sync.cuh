@@ -4,6 +4,19 @@
 #pragma once
 #include "reduce.cuh"
 
+// System-scope fences of the protocol.  LQCD_SLAB_FENCE_EXPERIMENT (a bit mask, measurement only, never
+// set in a build that talks to another GPU) narrows fence i to device scope to time what each one costs.
+#ifndef LQCD_SLAB_FENCE_EXPERIMENT
+#define LQCD_SLAB_FENCE_EXPERIMENT 0
+#endif
+#define LQCD_SLAB_FENCE(bit)                                   \
+    do {                                                       \
+        if (LQCD_SLAB_FENCE_EXPERIMENT & (bit))                \
+            __threadfence();                                   \
+        else                                                   \
+            __threadfence_system();                            \
+    } while (0)
+
 namespace lqcd {
 
 constexpr int kSlabMaxRanks = 16;
@@ -55,7 +68,7 @@ __device__ __forceinline__ void slab_signal(const SlabSyncArgs& a, unsigned long
 {
     double* dst = a.peer_slot[r] + ((seq & 1ull) * a.nranks + a.rank) * 2;
     for (int k = 0; k < a.nvals; ++k) dst[k] = a.ss->part[k];
-    __threadfence_system();
+    LQCD_SLAB_FENCE(1);
     *(volatile unsigned long long*)(a.peer_flag[r] + a.rank) = seq;
 }
 
@@ -88,7 +101,7 @@ __device__ __forceinline__ void slab_combine(const SlabSyncArgs& a, unsigned lon
         a.sc->done = 1;
         return;
     }
-    __threadfence_system();
+    LQCD_SLAB_FENCE(2);
     double total[2] = { 0.0, 0.0 };
     const volatile double* s = a.own.slot + (seq & 1ull) * a.nranks * 2;
     for (int q = 0; q < a.nranks; ++q)
