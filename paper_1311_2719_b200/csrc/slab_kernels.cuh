@@ -1,6 +1,6 @@
 // slab_kernels.cuh -- kernels of the time-slab decomposition (
 // include/lqcd_slab.h) that are not Dslash: the vector kernels with the face stores fused in,
-// and the two tiny kernels of a cross-rank synchronisation point.
+// and the stand-alone kernels of a cross-rank synchronisation point (slab_sync.cuh has its pieces).
 //
 // A synchronisation point, number `seq` (1, 2, 3, ... since lqcd_slab_connect, the same on every rank
 // because every rank makes the same sequence of calls):
@@ -13,7 +13,9 @@
 //                     thread adds the slots in RANK ORDER -- every rank adds the same numbers in the
 //                     same order, so all ranks hold bit-identical scalars and take the same exit
 //                     decision -- and runs the scalar step of the CG.
-//   (a rank that drives only its own slab runs signal and wait_combine as one launch.)
+//   A rank that drives only its own slab runs signal + wait + combine in the LAST BLOCK of the producer
+//   kernel (slab_sync_tail; no extra launch), or as one launch after producers that have no sum; a group
+//   of slabs on one stream launches all signals, then all waits, so that no kernel ever spins.
 // Buffers alternate with seq & 1: a rank can be at most one synchronisation point ahead of a peer
 // that has not read its faces/slots yet, never two (it needs that peer's next signal to go on).
 // The paper instead gathers the WHOLE vector through the host every iteration.
