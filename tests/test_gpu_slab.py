@@ -271,6 +271,46 @@ def test_slab_edge_cases_and_errors(sl):
         s.close()
 
 
+@pytest.mark.parametrize("nranks", [1, 4])
+def test_slab_cg_cfg3_bench_workload(sl, nranks):
+    """32^4, m = 0.01 as `bench.py --parallelism slab` times it (nranks = 1: lqcd_slab_cg_solve with the fused
+    synchronisation tail and graph replay) and cut into four slabs.  The oracle's own solve takes minutes:
+    its stored iteration count and sampled solution entries (tests/golden, written by make_golden.py from
+    oracle/ alone) and one oracle application of A to the assembled solution are the references."""
+    import json
+    import os
+    golden = os.path.join(os.path.dirname(__file__), "golden", "oracle_cg_reference.json")
+    if not os.path.exists(golden) or "cfg3" not in json.load(open(golden)):
+        pytest.skip("no stored oracle reference for cfg3")
+    ref = json.load(open(golden))["cfg3"]
+    c, u, b = synth.config_inputs(3)
+    dims = c["dims"]
+    if nranks == 1:
+        ug = torch.from_numpy(u)
+        s = sl.Slab(dims, 0, 1)
+        try:
+            s.connect([s.mailbox_ptr])
+            s.load_gauge(sl.local_gauge(ug, dims, 0, 1).cuda(), sl.u3_below_from_global(ug, dims, 0, 1).cuda())
+            xt, it, res, status = s.cg_solve(c["param"], c["tol"], 50000, torch.from_numpy(b).cuda(), s.new_vector())
+            x = xt.cpu().numpy()
+        finally:
+            s.close()
+    else:
+        g = group_for(sl, dims, nranks, u)
+        try:
+            xs, it, res, status = g.cg_solve(c["param"], c["tol"], 50000, g.scatter(torch.from_numpy(b)), g.new_vectors())
+            x = gathered(sl, xs)
+        finally:
+            g.close()
+    assert status == 0 and res <= 2 * c["tol"] and abs(it - ref["iters"]) <= 2
+    idx = np.asarray(ref["sample_index"])
+    want = np.asarray(ref["sample_re"]) + 1j * np.asarray(ref["sample_im"])
+    assert np.linalg.norm(x.ravel()[idx] - want) <= CG_TOL * ref["x_norm"] * np.sqrt(len(idx) / x.size) * 10
+    assert abs(np.linalg.norm(x.ravel()) - ref["x_norm"]) <= CG_TOL * ref["x_norm"]
+    ax = oracle.apply_MdagM(dims, 0, u, c["param"], x)
+    assert abs(rel(ax, b) - res) <= 1e-3 * res + 1e-13
+
+
 # ------------------------------------------------------------------ CUDA IPC plumbing, two processes on the one GPU
 def _ipc_worker(rank, world, port, out):
     """Maps the peer's mailbox through lqcd_slab_ipc_export / _open and moves bytes with plain copies.
