@@ -164,16 +164,37 @@ StagArgsD stag_args(const lqcd_ctx* ctx, int parity, const cplx* in, cplx* out)
     return a;
 }
 
+// Threads per block of the fp64 staggered kernels.  128 on lattices that fill the machine; small lattices
+// are latency-bound and gain from more, smaller blocks (B200, us per CG iteration / plain Dslash at
+// 128, 64, 32 threads: 16^4 30.4 / 10.3, 27.2 / 7.3, 25.9 / 6.3; 4^4 20.7 / 6.2, 18.7 / 4.6, 17.1 / 4.2;
+// 32^4 234.9, 242.6, 267.3 per iteration: profiles/r01_bench.md).
+int stag_block_for(const lqcd_ctx* ctx)
+{
+    const long long blocks128 = ((long long)ctx->g.Vh + 127) / 128;
+    if (blocks128 < 2 * 148) return 32;
+    if (blocks128 < 8 * 148) return 64;
+    return 128;
+}
+
+template <int EPI, int BLOCK>
+int launch_stag_block(lqcd_ctx* ctx, const StagArgsD& a)
+{
+    const unsigned int grid = blocks_for(ctx->g.Vh, BLOCK);
+    if (ctx->recon == 12)
+        stag_dslash_kernel<EPI, BLOCK, 12, cplx><<<grid, BLOCK, 0, ctx->stream>>>(a);
+    else
+        stag_dslash_kernel<EPI, BLOCK, 18, cplx><<<grid, BLOCK, 0, ctx->stream>>>(a);
+    LQCD_LAUNCH_CHECK();
+    return LQCD_OK;
+}
+
 template <int EPI>
 int launch_stag(lqcd_ctx* ctx, const StagArgsD& a)
 {
-    const unsigned int grid = blocks_for(ctx->g.Vh, kStagBlock);
-    if (ctx->recon == 12)
-        stag_dslash_kernel<EPI, kStagBlock, 12, cplx><<<grid, kStagBlock, 0, ctx->stream>>>(a);
-    else
-        stag_dslash_kernel<EPI, kStagBlock, 18, cplx><<<grid, kStagBlock, 0, ctx->stream>>>(a);
-    LQCD_LAUNCH_CHECK();
-    return LQCD_OK;
+    const int block = stag_block_for(ctx);
+    if (block == 32) return launch_stag_block<EPI, 32>(ctx, a);
+    if (block == 64) return launch_stag_block<EPI, 64>(ctx, a);
+    return launch_stag_block<EPI, kStagBlock>(ctx, a);
 }
 
 // fp32 instantiations: only the two kernels of the inner iteration of the mixed-precision solver
