@@ -193,29 +193,55 @@ StagArgsD stag_args(const lqcd_slab* s, int parity, const cplx* in, cplx* out, b
     return a;
 }
 
+// Threads per block by the size of the LOCAL lattice, as stag_block_for in lqcd_api.cu: strong scaling
+// shrinks the slabs, and small lattices want more, smaller blocks.
+int slab_block_for(const lqcd_slab* s)
+{
+    const long long blocks128 = ((long long)s->g.Vh + 127) / 128;
+    if (blocks128 < 2 * 148) return 32;
+    if (blocks128 < 8 * 148) return 64;
+    return 128;
+}
+
+template <int EPI, int BLOCK>
+int launch_stag_block(lqcd_slab* s, const StagArgsD& a, const SlabSyncArgs* sy)
+{
+    const unsigned int grid = blocks_for(s->g.Vh, BLOCK);
+    if (sy) {  // the synchronisation point that follows runs in the kernel's last block
+        if (s->recon == 12)
+            stag_dslash_slab_sync_kernel<EPI, BLOCK, 12, cplx><<<grid, BLOCK, 0, s->stream>>>(a, *sy);
+        else
+            stag_dslash_slab_sync_kernel<EPI, BLOCK, 18, cplx><<<grid, BLOCK, 0, s->stream>>>(a, *sy);
+    } else {
+        if (s->recon == 12)
+            stag_dslash_slab_kernel<EPI, BLOCK, 12, cplx><<<grid, BLOCK, 0, s->stream>>>(a);
+        else
+            stag_dslash_slab_kernel<EPI, BLOCK, 18, cplx><<<grid, BLOCK, 0, s->stream>>>(a);
+    }
+    SLAB_LAUNCH_CHECK();
+    return LQCD_OK;
+}
+
+template <int EPI>
+int launch_stag_any(lqcd_slab* s, const StagArgsD& a, const SlabSyncArgs* sy)
+{
+    const int block = slab_block_for(s);
+    if (block == 32) return launch_stag_block<EPI, 32>(s, a, sy);
+    if (block == 64) return launch_stag_block<EPI, 64>(s, a, sy);
+    return launch_stag_block<EPI, kStagBlock>(s, a, sy);
+}
+
 template <int EPI>
 int launch_stag(lqcd_slab* s, const StagArgsD& a)
 {
-    const unsigned int grid = blocks_for(s->g.Vh, kStagBlock);
-    if (s->recon == 12)
-        stag_dslash_slab_kernel<EPI, kStagBlock, 12, cplx><<<grid, kStagBlock, 0, s->stream>>>(a);
-    else
-        stag_dslash_slab_kernel<EPI, kStagBlock, 18, cplx><<<grid, kStagBlock, 0, s->stream>>>(a);
-    SLAB_LAUNCH_CHECK();
-    return LQCD_OK;
+    return launch_stag_any<EPI>(s, a, nullptr);
 }
 
 // The same kernel with the synchronisation point that follows it run by its last block.
 template <int EPI>
 int launch_stag_sync(lqcd_slab* s, const StagArgsD& a, const SlabSyncArgs& sy)
 {
-    const unsigned int grid = blocks_for(s->g.Vh, kStagBlock);
-    if (s->recon == 12)
-        stag_dslash_slab_sync_kernel<EPI, kStagBlock, 12, cplx><<<grid, kStagBlock, 0, s->stream>>>(a, sy);
-    else
-        stag_dslash_slab_sync_kernel<EPI, kStagBlock, 18, cplx><<<grid, kStagBlock, 0, s->stream>>>(a, sy);
-    SLAB_LAUNCH_CHECK();
-    return LQCD_OK;
+    return launch_stag_any<EPI>(s, a, &sy);
 }
 
 int launch_push_faces(lqcd_slab* s, const cplx* v)
