@@ -266,8 +266,6 @@ def main():
                     help="N > 1: replicas = independent right-hand sides per GPU (weak scaling, the default); "
                          "slab = ONE system cut into time-slabs, halo exchange and sums through peer memory "
                          "(strong scaling; include/lqcd_slab.h; staggered configs)")
-    ap.add_argument("--pdl", type=int, default=0, choices=[0, 1],
-                    help="1 = programmatic dependent launch of the kernels of the CG chain (LQCD_OPT_PDL)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -324,7 +322,6 @@ def main():
     lat.set_option(lqcd.OPT_CG_MODE, {"sync": lqcd.CG_SYNC, "async": lqcd.CG_ASYNC, "graph": lqcd.CG_GRAPH}[args.cg_mode])
     lat.set_option(lqcd.OPT_CG_CHECK_EVERY, args.check_every)
     lat.set_option(lqcd.OPT_RECONSTRUCT, args.recon)
-    lat.set_option(lqcd.OPT_PDL, args.pdl)
     u_dev = u_host.to(device, non_blocking=True)
     b_dev = b_host.to(device, non_blocking=True)
     lat.load_gauge(u_dev)
@@ -479,7 +476,7 @@ def main():
             "warmup": max(args.warmup, 3), "ms_per_step": ms_solve, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64" if not mixed else "f32 iterations + f64 reliable updates",
             "data": "synthetic",
-            "config": {"workload": workload, "precision": args.precision, "reconstruct": args.recon, "cg_mode": args.cg_mode, "check_every": args.check_every, "pdl": args.pdl,
+            "config": {"workload": workload, "precision": args.precision, "reconstruct": args.recon, "cg_mode": args.cg_mode, "check_every": args.check_every,
                        "parallelism": "replicas x%d (independent right-hand sides)" % world,
                        "l2_policy": "inputs larger than L2 (%.0f MB of links per Dslash), no flush" % (v * 576 / 1e6)},
             "cg": {"time_to_solution_ms": ms_solve, "iters": iters, "reliable_updates": updates if mixed else None,

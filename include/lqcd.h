@@ -90,12 +90,7 @@ enum {
      * read them with 128-bit loads (lattices with L0 % 4 == 0; others use the one-site kernels).
      * 0: one site per thread.  The vectors are bit-identical either way; the partial sums are
      * grouped differently, so scalars differ in the last bits. */
-    LQCD_OPT_F32_PAIRS = 4,
-    /* 1: the staggered Dslash and p-update kernels are launched with programmatic dependent launch
-     * (the next kernel is scheduled while the previous one drains and waits on the device for its
-     * completion before reading anything): same kernels, same order, bit-identical results; hides
-     * launch latency between the three kernels of an iteration.  0: plain stream order. */
-    LQCD_OPT_PDL = 5
+    LQCD_OPT_F32_PAIRS = 4
 };
 
 /* Create a context for an L0 x L1 x L2 x L3 lattice (every extent even and >= 2; L = 2 is

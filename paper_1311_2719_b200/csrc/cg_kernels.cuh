@@ -130,7 +130,6 @@ template <int BLOCK, class C>
 __global__ void __launch_bounds__(BLOCK) cg_pupdate_kernel(const C* __restrict__ r, C* __restrict__ p, VecLayout lay,
                                                            CgScalars* sc, ReduceScratch rs)
 {
-    pdl_wait();
     if (sc->done | sc->pause) return;
     const double beta = sc->beta;
     double local = 0.0;
@@ -144,7 +143,6 @@ __global__ void __launch_bounds__(BLOCK) cg_pupdate_kernel(const C* __restrict__
         p[i] = ps;
         local += cnorm2(ps);
     }
-    pdl_launch_dependents();
     grid_sum<BLOCK>(local, rs, [sc](double pp) { sc->pp = pp; });
 }
 

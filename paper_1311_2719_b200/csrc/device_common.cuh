@@ -83,16 +83,6 @@ __device__ __forceinline__ double half_eta(const Site& s)
     return ((s.r + s.x1 + s.x2) & 1) ? -0.5 : 0.5;
 }
 
-// ------------------------------------------------------------------ programmatic dependent launch
-// The kernels of a CG iteration are launched with cudaLaunchAttributeProgrammaticStreamSerialization
-// (LQCD_OPT_PDL): the next kernel's blocks may be scheduled while this one drains, which hides the launch
-// latency and the ramp of the three short kernels per iteration.  pdl_wait() must precede the first
-// access to anything an earlier kernel wrote (it returns once that kernel has completed and its
-// memory is visible; a no-op in a launch without the attribute); pdl_launch_dependents() says this
-// block no longer minds the next kernel's blocks sharing its SM.
-__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
-__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
-
 // ------------------------------------------------------------------ loads / stores
 // Links are read exactly once per Dslash and the field (0.6-6 GB) does not fit the 126 MB L2:
 // stream them (evict-first, no L1 allocation) so they do not push the vectors out.

@@ -57,7 +57,6 @@ struct lqcd_ctx {
     int recon;  // 18 or 12 stored reals per link
     int congrad_precision;  // 64 or 32: which solver lqcd_congrad_host runs
     int f32_pairs;          // fp32 kernels of the mixed solver: two sites per thread with 128-bit loads
-    int pdl;                // programmatic dependent launch of the kernels of the CG chain
     bool wilson_eo;  // set while lqcd_wilson_solve_eo runs: the CG works on Mhat^+ Mhat, even half of the vectors
     // host side
     CgScalars* h_sc;  // pinned, 2 slots
@@ -127,26 +126,6 @@ int check_ready(lqcd_ctx* ctx, bool need_gauge)
 
 unsigned int blocks_for(size_t n, int block) { return (unsigned int)((n + block - 1) / block); }
 
-// Launch of a kernel of the CG chain.  With LQCD_OPT_PDL the launch carries the programmatic-stream-
-// serialization attribute: the kernel may be scheduled while its predecessor drains (it calls pdl_wait()
-// before touching anything the predecessor wrote), which takes the launch latency and the ramp of the
-// three kernels per iteration off the critical path.  Captured into CUDA graphs like any launch.
-template <class... KArgs, class... Args>
-void launch_chain(lqcd_ctx* ctx, void (*kernel)(KArgs...), unsigned int grid, unsigned int block, Args&&... args)
-{
-    cudaLaunchConfig_t cfg;
-    memset(&cfg, 0, sizeof cfg);
-    cfg.gridDim = dim3(grid);
-    cfg.blockDim = dim3(block);
-    cfg.stream = ctx->stream;
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    at[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = at;
-    cfg.numAttrs = ctx->pdl ? 1 : 0;
-    cudaLaunchKernelEx(&cfg, kernel, static_cast<Args&&>(args)...);  // errors surface in LQCD_LAUNCH_CHECK
-}
-
 VecLayout vec_layout(const lqcd_ctx* ctx)
 {
     VecLayout l;
@@ -202,9 +181,9 @@ int launch_stag_block(lqcd_ctx* ctx, const StagArgsD& a)
 {
     const unsigned int grid = blocks_for(ctx->g.Vh, BLOCK);
     if (ctx->recon == 12)
-        launch_chain(ctx, stag_dslash_kernel<EPI, BLOCK, 12, cplx>, grid, BLOCK, a);
+        stag_dslash_kernel<EPI, BLOCK, 12, cplx><<<grid, BLOCK, 0, ctx->stream>>>(a);
     else
-        launch_chain(ctx, stag_dslash_kernel<EPI, BLOCK, 18, cplx>, grid, BLOCK, a);
+        stag_dslash_kernel<EPI, BLOCK, 18, cplx><<<grid, BLOCK, 0, ctx->stream>>>(a);
     LQCD_LAUNCH_CHECK();
     return LQCD_OK;
 }
@@ -240,17 +219,17 @@ int launch_stag_f(lqcd_ctx* ctx, const StagArgsF& a)
     if (ctx->f32_pairs && ctx->g.Lh % 2 == 0) {  // two sites per thread, 128-bit loads (stag_dslash_f32x2.cuh)
         const unsigned int grid2 = blocks_for((size_t)ctx->g.Vh / 2, kStagBlock);
         if (ctx->recon == 12)
-            launch_chain(ctx, stag_dslash_f32x2_kernel<EPI, kStagBlock, 12>, grid2, kStagBlock, a);
+            stag_dslash_f32x2_kernel<EPI, kStagBlock, 12><<<grid2, kStagBlock, 0, ctx->stream>>>(a);
         else
-            launch_chain(ctx, stag_dslash_f32x2_kernel<EPI, kStagBlock, 18>, grid2, kStagBlock, a);
+            stag_dslash_f32x2_kernel<EPI, kStagBlock, 18><<<grid2, kStagBlock, 0, ctx->stream>>>(a);
         LQCD_LAUNCH_CHECK();
         return LQCD_OK;
     }
     const unsigned int grid = blocks_for(ctx->g.Vh, kStagBlock);
     if (ctx->recon == 12)
-        launch_chain(ctx, stag_dslash_kernel<EPI, kStagBlock, 12, cplxf>, grid, kStagBlock, a);
+        stag_dslash_kernel<EPI, kStagBlock, 12, cplxf><<<grid, kStagBlock, 0, ctx->stream>>>(a);
     else
-        launch_chain(ctx, stag_dslash_kernel<EPI, kStagBlock, 18, cplxf>, grid, kStagBlock, a);
+        stag_dslash_kernel<EPI, kStagBlock, 18, cplxf><<<grid, kStagBlock, 0, ctx->stream>>>(a);
     LQCD_LAUNCH_CHECK();
     return LQCD_OK;
 }
@@ -348,8 +327,8 @@ int cg_iteration_kernels(lqcd_ctx* ctx, double param, cplx* x)
 
 int cg_pupdate(lqcd_ctx* ctx)  // S5
 {
-    launch_chain(ctx, cg_pupdate_kernel<kVecBlock, cplx>, vec_grid(ctx), kVecBlock, ctx->r(), ctx->p(), vec_layout(ctx), ctx->sc(),
-                 ctx->rs());
+    cg_pupdate_kernel<kVecBlock, cplx><<<vec_grid(ctx), kVecBlock, 0, ctx->stream>>>(ctx->r(), ctx->p(), vec_layout(ctx), ctx->sc(),
+                                                                              ctx->rs());
     LQCD_LAUNCH_CHECK();
     return LQCD_OK;
 }
@@ -494,13 +473,13 @@ int mixed_iteration_kernels(lqcd_ctx* ctx, double mass)  // S1 + S2, S3 on the f
 int mixed_pupdate(lqcd_ctx* ctx)  // S5 on the fp32 copies
 {
     if (ctx->f32_pairs && ctx->nvec % 2 == 0) {
-        launch_chain(ctx, cg_pupdate_f32x2_kernel<kVecBlock>, vec_grid(ctx), kVecBlock, ctx->rf(), ctx->pf(), ctx->nvec, ctx->sc(),
-                     ctx->rs());
+        cg_pupdate_f32x2_kernel<kVecBlock><<<vec_grid(ctx), kVecBlock, 0, ctx->stream>>>(ctx->rf(), ctx->pf(), ctx->nvec, ctx->sc(),
+                                                                                       ctx->rs());
         LQCD_LAUNCH_CHECK();
         return LQCD_OK;
     }
-    launch_chain(ctx, cg_pupdate_kernel<kVecBlock, cplxf>, vec_grid(ctx), kVecBlock, ctx->rf(), ctx->pf(), vec_layout(ctx), ctx->sc(),
-                 ctx->rs());
+    cg_pupdate_kernel<kVecBlock, cplxf><<<vec_grid(ctx), kVecBlock, 0, ctx->stream>>>(ctx->rf(), ctx->pf(), vec_layout(ctx),
+                                                                                      ctx->sc(), ctx->rs());
     LQCD_LAUNCH_CHECK();
     return LQCD_OK;
 }
@@ -640,7 +619,6 @@ int lqcd_create(lqcd_ctx** out, int L0, int L1, int L2, int L3, int fermion_type
     c->recon = 18;
     c->congrad_precision = 64;
     c->f32_pairs = 1;
-    c->pdl = 0;
 
     size_t off = 0;
     const size_t vec_bytes = align_up(c->nvec * sizeof(cplx));
@@ -730,11 +708,6 @@ int lqcd_set_option(lqcd_ctx* ctx, int option, int value)
         if (value != 64 && !(value == 32 && ctx->fermion == LQCD_STAGGERED))
             return fail(ctx, LQCD_EARG, "congrad precision must be 64, or 32 on a staggered context");
         ctx->congrad_precision = value;
-        return LQCD_OK;
-    }
-    if (option == LQCD_OPT_PDL) {
-        if (value != 0 && value != 1) return fail(ctx, LQCD_EARG, "pdl must be 0 or 1");
-        ctx->pdl = value;
         return LQCD_OK;
     }
     if (option == LQCD_OPT_F32_PAIRS) {

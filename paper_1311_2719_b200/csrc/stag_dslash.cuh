@@ -181,7 +181,6 @@ __device__ __forceinline__ void slab_push(const StagArgs<C>& a, int x3, int e, c
 template <int EPI, int BLOCK, int RECON, bool SLAB, class C>
 __device__ __forceinline__ void stag_dslash_body(const StagArgs<C>& a, const SlabSyncArgs* sy = nullptr)
 {
-    pdl_wait();
     if (EPI == SE_NORM || EPI == SE_CGUPDATE || EPI == SE_CGUPDATE_MIXED) {
         // converged earlier, or waiting for a reliable update: this (pre-enqueued) iteration is a no-op
         if (a.sc->done | a.sc->pause) return;
@@ -199,7 +198,6 @@ __device__ __forceinline__ void stag_dslash_body(const StagArgs<C>& a, const Sla
         stag_hop<2, RECON, SLAB>(a, s, acc);
         stag_hop<3, RECON, SLAB>(a, s, acc);
     }
-    pdl_launch_dependents();
     bool wrote_peer = false;
     if (SLAB && (EPI == SE_PLAIN || EPI == SE_NORM)) {
         if (active) {

@@ -105,7 +105,6 @@ template <int EPI, int BLOCK, int RECON>
 __global__ void __launch_bounds__(BLOCK, LQCD_STAG_MINB_F32X2) stag_dslash_f32x2_kernel(const StagArgs<cplxf> a)
 {
     static_assert(EPI == SE_NORM || EPI == SE_CGUPDATE_MIXED, "only the two kernels of the fp32 iteration");
-    pdl_wait();
     if (a.sc->done | a.sc->pause) return;
     const int e = 2 * (blockIdx.x * BLOCK + threadIdx.x);
     const bool active = e < a.g.Vh;
@@ -122,7 +121,6 @@ __global__ void __launch_bounds__(BLOCK, LQCD_STAG_MINB_F32X2) stag_dslash_f32x2
         stag_hop2<2, RECON>(a, s, acc);
         stag_hop2<3, RECON>(a, s, acc);
     }
-    pdl_launch_dependents();
     double local = 0.0;
     if (EPI == SE_NORM) {
         if (active) {
@@ -177,7 +175,6 @@ template <int BLOCK>
 __global__ void __launch_bounds__(BLOCK) cg_pupdate_f32x2_kernel(const cplxf* __restrict__ r, cplxf* __restrict__ p, size_t n,
                                                                  CgScalars* sc, ReduceScratch rs)
 {
-    pdl_wait();
     if (sc->done | sc->pause) return;
     const double beta = sc->beta;
     double local = 0.0;
@@ -197,7 +194,6 @@ __global__ void __launch_bounds__(BLOCK) cg_pupdate_f32x2_kernel(const cplxf* __
         }
         *(float4*)(p + 2 * j) = join(p2[0], p2[1]);
     }
-    pdl_launch_dependents();
     grid_sum<BLOCK>(local, rs, [sc](double pp) { sc->pp = pp; });
 }
 

@@ -181,27 +181,6 @@ def test_cg_modes_give_identical_iterates(lq):
         assert it2 == it0 and res2 == res0 and np.array_equal(x0, x2)
 
 
-@pytest.mark.parametrize("cfg", [1, 2])
-def test_cg_programmatic_dependent_launch_changes_no_bit(lq, cfg):
-    """LQCD_OPT_PDL: the same kernels in the same order, each scheduled while its predecessor drains."""
-    c, u, b = synth.config_inputs(cfg)
-    with make_lattice(lq, c["dims"], 0, u) as lat:
-        ref = None
-        for pdl in (0, 1):
-            lat.set_option(lq.OPT_PDL, pdl)
-            for mode in (lq.CG_SYNC, lq.CG_ASYNC, lq.CG_GRAPH):
-                x, it, res, status = run_cg(lat, c, b, mode=mode)
-                got = (x, it, res, status, lat.cg_history().numpy())
-                if ref is None:
-                    ref = got
-                assert got[1:4] == ref[1:4] and np.array_equal(got[0], ref[0]) and np.array_equal(got[4], ref[4])
-            xm, itm, num, resm, stm = lat.cg_solve_mixed(c["param"], c["tol"], 20000, dev(b))
-            if pdl == 0:
-                mixed_ref = (xm.cpu().numpy(), itm, num, resm)
-            else:
-                assert (itm, num, resm) == mixed_ref[1:] and np.array_equal(xm.cpu().numpy(), mixed_ref[0])
-
-
 @pytest.mark.parametrize("mode", [0, 1, 2])
 def test_cg_fixed_iteration_count_matches_oracle_iterate(lq, mode):
     """tol = 0 runs exactly maxiter iterations: compare the iterate x_k itself."""
