@@ -311,6 +311,34 @@ def test_slab_cg_cfg3_bench_workload(sl, nranks):
     assert abs(rel(ax, b) - res) <= 1e-3 * res + 1e-13
 
 
+@pytest.mark.slow
+def test_slab_cg_cfg5_eight_slabs(sl):
+    """48^3 x 96 (6 GB of links) cut into eight slabs of 12 time-slices, as an 8-GPU run would hold it: the
+    assembled solution against one oracle application of A (holds at any size) and, where stored, the
+    oracle's iteration count and sampled solution entries."""
+    import json
+    import os
+    c, u, b = synth.config_inputs(5)
+    dims = c["dims"]
+    g = group_for(sl, dims, 8, u)
+    try:
+        xs, it, res, status = g.cg_solve(c["param"], c["tol"], 50000, g.scatter(torch.from_numpy(b)), g.new_vectors())
+        x = gathered(sl, xs)
+    finally:
+        g.close()
+    assert status == 0 and res <= 2 * c["tol"]
+    ax = oracle.apply_MdagM(dims, 0, u, c["param"], x)
+    assert abs(rel(ax, b) - res) <= 1e-3 * res + 1e-13
+    golden = os.path.join(os.path.dirname(__file__), "golden", "oracle_cg_reference.json")
+    if os.path.exists(golden) and "cfg5" in json.load(open(golden)):
+        ref = json.load(open(golden))["cfg5"]
+        assert abs(it - ref["iters"]) <= 2
+        idx = np.asarray(ref["sample_index"])
+        want = np.asarray(ref["sample_re"]) + 1j * np.asarray(ref["sample_im"])
+        assert np.linalg.norm(x.ravel()[idx] - want) <= CG_TOL * ref["x_norm"] * np.sqrt(len(idx) / x.size) * 10
+        assert abs(np.linalg.norm(x.ravel()) - ref["x_norm"]) <= CG_TOL * ref["x_norm"]
+
+
 # ------------------------------------------------------------------ CUDA IPC plumbing, two processes on the one GPU
 def _ipc_worker(rank, world, port, out):
     """Maps the peer's mailbox through lqcd_slab_ipc_export / _open and moves bytes with plain copies.
