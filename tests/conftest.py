@@ -25,3 +25,11 @@ def _built_library():
     """The CUDA library is built in-tree (nvcc cross-compiles without a GPU)."""
     from paper_1311_2719_b200 import build
     build.build()
+
+
+@pytest.fixture(scope="session")
+def cfg5_inputs():
+    """(cfg, gauge field, source) of BASELINE.json config 5 (48^3 x 96, 6 GB of links): generated once
+    per session, the three full-size tests share it."""
+    from paper_1311_2719_b200 import synth
+    return synth.config_inputs(5)

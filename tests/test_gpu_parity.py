@@ -116,10 +116,10 @@ def test_dslash_configs_full_comparison(lq, cfg, recon):
 
 
 @pytest.mark.slow
-def test_dslash_cfg5_sampled_sites_and_norm(lq):
+def test_dslash_cfg5_sampled_sites_and_norm(lq, cfg5_inputs):
     """48^3 x 96 (6 GB of links): the oracle computes 4096 sampled output sites one by one; the
     rest is covered by anti-hermiticity, <phi, D chi> = -<D phi, chi>, which holds at any size."""
-    c, u, b = synth.config_inputs(5)
+    c, u, b = cfg5_inputs
     dims = c["dims"]
     vh = synth.volume(dims) // 2
     rng = np.random.default_rng(55)
@@ -291,8 +291,8 @@ def test_cg_cfg3_bench_workload(lq, recon):
 
 
 @pytest.mark.slow
-def test_cg_cfg5(lq):
-    c, u, b = synth.config_inputs(5)
+def test_cg_cfg5(lq, cfg5_inputs):
+    c, u, b = cfg5_inputs
     with make_lattice(lq, c["dims"], 0, u) as lat:
         x, it, res, status = run_cg(lat, c, b, maxiter=50000)
     assert status == 0 and res <= 2 * c["tol"]

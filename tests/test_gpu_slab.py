@@ -312,13 +312,13 @@ def test_slab_cg_cfg3_bench_workload(sl, nranks):
 
 
 @pytest.mark.slow
-def test_slab_cg_cfg5_eight_slabs(sl):
+def test_slab_cg_cfg5_eight_slabs(sl, cfg5_inputs):
     """48^3 x 96 (6 GB of links) cut into eight slabs of 12 time-slices, as an 8-GPU run would hold it: the
     assembled solution against one oracle application of A (holds at any size) and, where stored, the
     oracle's iteration count and sampled solution entries."""
     import json
     import os
-    c, u, b = synth.config_inputs(5)
+    c, u, b = cfg5_inputs
     dims = c["dims"]
     g = group_for(sl, dims, 8, u)
     try:
