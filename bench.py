@@ -12,8 +12,10 @@ kernel (1248 B per output site) timed with CUDA events on the library's stream.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1..5]
 
-N > 1 (torchrun): replicas only -- every rank solves its own right-hand side on the same gauge
-field, no data-path collective; scaling = weak.
+N > 1 (torchrun): by default replicas -- every rank solves its own right-hand side on the same gauge
+field, no data-path collective; scaling = weak.  --parallelism slab: ONE system cut
+into time-slabs, one per GPU (include/lqcd_slab.h: halo stores and sums through peer memory); scaling =
+strong; not yet timed on more than one GPU.
 """
 from __future__ import annotations
 

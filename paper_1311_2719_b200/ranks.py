@@ -1,7 +1,8 @@
 """One process per GPU: the rank plumbing bench.py and the multi-rank drivers share.
 
 The path of arXiv 1311.2719 runs on one GPU (BASELINE.json); with N > 1 processes every rank
-owns independent right-hand sides on the same gauge field ("replicas only"):
+owns independent right-hand sides on the same gauge field (the replicas mode of DESIGN.md section 8;
+the time-slab decomposition of one system lives in slab.py and include/lqcd_slab.h):
 no data-path collective, only the timing reductions below.  `torch.distributed` is the
 transport: NCCL on GPUs, gloo in the CPU tests (world_size 2, 127.0.0.1).
 
