@@ -312,14 +312,62 @@ def test_cg_recursion_residual_matches_true_residual_cfg1():
     assert abs(h[0] - bb) < 1e-12 * bb
     assert h[-1] <= c["tol"] ** 2 * bb < h[-2]
     rec = np.sqrt(h[-1] / bb)
-    assert abs(rec - r["true_residual"]) < 1e-8 * 1.0 and r["true_residual"] < 2e-10
+    assert abs(rec - r["true_residual"]) < 1e-3 * r["true_residual"] and r["true_residual"] < 2e-10
     # the solution satisfies the equation as checked with numpy on the oracle's operator output
     ax = oracle.apply_MdagM(c["dims"], STAGGERED, u, c["param"], r["x"])
     assert rel(ax, b) < 2e-10
 
 
-def test_thread_count_does_not_change_results():
-    c, u, b = synth.config_inputs(1)
+@pytest.mark.parametrize("fermion", [STAGGERED, WILSON])
+def test_cg_true_residual_is_the_fresh_residual(fermion):
+    """`true_residual` is |b - A x| / |b| with a FRESH application of A (SURVEY 8(c.4) last line; the
+    exit test itself, uses the recursion's <r,r>).  The norm is retaken here in numpy
+    from the oracle's operator output; the two agree to summation-order rounding (1e-12 relative), while
+    the recursion's value is measurably different after a few hundred iterations -- so a residual
+    reported from the recursion, a missing sqrt, or a division by <r,r> instead of <b,b> fails."""
+    if fermion == STAGGERED:
+        c, u, b = synth.config_inputs(1)
+        dims, param = c["dims"], c["param"]
+    else:
+        dims, param = (4, 4, 4, 4), 0.12
+        u = synth.gauge_field(dims, "smooth", 5)
+        b = synth.source(dims, "wilson", 6)
+    r = oracle.cg(dims, fermion, u, param, 1e-10, 5000, b, history=True)
+    assert r["status"] == 0
+    ax = oracle.apply_MdagM(dims, fermion, u, param, r["x"])
+    fresh = np.linalg.norm((b - ax).ravel()) / np.linalg.norm(b.ravel())
+    assert abs(fresh - r["true_residual"]) <= 1e-12 * fresh
+    rec = np.sqrt(r["rr_history"][-1] / vdot(b, b).real)
+    assert abs(rec - fresh) > 1e-8 * fresh        # the pin above can tell the two apart ...
+    assert abs(rec - fresh) < 1e-3 * fresh        # ... and the recursion has not drifted (P9)
+    # a MAXITER exit reports the residual of the iterate it returns, not of a converged one
+    r7 = oracle.cg(dims, fermion, u, param, 1e-10, 7, b)
+    ax7 = oracle.apply_MdagM(dims, fermion, u, param, r7["x"])
+    fresh7 = np.linalg.norm((b - ax7).ravel()) / np.linalg.norm(b.ravel())
+    assert r7["status"] == 1 and fresh7 > 1e-3 and abs(fresh7 - r7["true_residual"]) <= 1e-12 * fresh7
+
+
+def test_dot_re_over_several_blocks_and_a_ragged_tail():
+    """oracle.dot_re sums in fixed 4096-element blocks; n = 3 blocks + 17 exercises the block loop and
+    the tail (a dropped tail block or a wrong block bound changes the sum by O(1))."""
+    rng = np.random.default_rng(1311)
+    for n in (1, 17, 4096, 4097, 3 * 4096 + 17):
+        a = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+        b = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+        want = np.vdot(a, b).real
+        scale = np.linalg.norm(a) * np.linalg.norm(b)
+        assert abs(oracle.dot_re(a, b) - want) <= 1e-14 * scale
+        assert abs(oracle.dot_re(a, a) - np.linalg.norm(a) ** 2) <= 1e-14 * scale
+    # Re<a,b> = Re conj(a).b: conjugation on the FIRST argument, real part only
+    a = np.array([1 + 2j, 3 - 1j]); b = np.array([2 - 1j, 1j])
+    assert oracle.dot_re(a, b) == (np.conj(a) * b).sum().real == -1.0
+
+
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_thread_count_does_not_change_results(cfg):
+    """cfg 1: 384 elements = one block of the blocked dot product; cfg 2: 98 304 elements = 24 blocks
+    shared out between the threads -- the path every 16^4 and larger CG takes."""
+    c, u, b = synth.config_inputs(cfg)
     n0 = oracle.num_threads()
     try:
         oracle.set_threads(1)
