@@ -33,3 +33,19 @@ def cfg5_inputs():
     per session, the three full-size tests share it."""
     from paper_1311_2719_b200 import synth
     return synth.config_inputs(5)
+
+
+@pytest.fixture(scope="session")
+def cfg3_inputs():
+    from paper_1311_2719_b200 import synth
+    return synth.config_inputs(3)
+
+
+@pytest.fixture(scope="session")
+def cfg3_oracle_cg(cfg3_inputs):
+    """The oracle's own CG on BASELINE.json config 3 (32^4, m = 0.01: 3138 iterations, about a minute on the
+    GPU box's 16 host cores), run ONCE per session: the full-size tests compare the WHOLE solution vector
+    with it at the north-star tolerance, not a sample."""
+    import oracle
+    c, u, b = cfg3_inputs
+    return oracle.cg(c["dims"], 0, u, c["param"], c["tol"], 100000, b)

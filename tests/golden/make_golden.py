@@ -24,6 +24,16 @@ import oracle  # noqa: E402
 from paper_1311_2719_b200 import synth  # noqa: E402
 
 OUT = os.path.join(os.path.dirname(os.path.abspath(__file__)), "oracle_cg_reference.json")
+
+
+def dump(ref):
+    """One key per line, number lists on one line (the 4096-entry samples stay readable in a diff)."""
+    lines = []
+    for name in sorted(ref):
+        items = ",\n".join('  %s: %s' % (json.dumps(k), json.dumps(ref[name][k])) for k in sorted(ref[name]))
+        lines.append(' %s: {\n%s\n }' % (json.dumps(name), items))
+    with open(OUT, "w") as f:
+        f.write("{\n" + ",\n".join(lines) + "\n}\n")
 NSAMPLE = 4096     # cfg 1, 2, 4 (re-run in full inside the GPU tests) were written with 64
 
 
@@ -42,7 +52,7 @@ def mixed(cfgs):
         }
         print("cfg%d mixed: iters %d, updates %d, true residual %.3e, %.1f s"
               % (n, r["iters"], r["updates"], r["true_residual"], dt), flush=True)
-        json.dump(ref, open(OUT, "w"), indent=1, sort_keys=True)
+        dump(ref)
 
 
 def main():
@@ -68,7 +78,7 @@ def main():
             "oracle_threads": oracle.num_threads(),
         }
         print("cfg%d: iters %d, true residual %.3e, %.1f s" % (n, r["iters"], r["true_residual"], dt), flush=True)
-        json.dump(ref, open(OUT, "w"), indent=1, sort_keys=True)
+        dump(ref)
 
 
 if __name__ == "__main__":

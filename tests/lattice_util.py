@@ -54,3 +54,32 @@ def read_gammas(path):
         gam[mu, row] = [val[t] for t in line.split()]
         row += 1
     return gam
+
+
+# ------------------------------------------------------------------ stored oracle references
+import json as _json
+import os as _os
+
+GOLDEN = _os.path.join(_os.path.dirname(_os.path.abspath(__file__)), "golden", "oracle_cg_reference.json")
+
+
+def golden(key):
+    """Entry `key` ("cfg3", "cfg5", "cfg3_mixed", ...) of tests/golden/oracle_cg_reference.json (written by
+    tests/golden/make_golden.py from oracle/ alone).  A missing file or entry FAILS the test: parity against
+    the oracle's CG is part of the contract on every BASELINE.json config."""
+    assert _os.path.exists(GOLDEN), "tests/golden/oracle_cg_reference.json is missing: run tests/golden/make_golden.py"
+    ref = _json.load(open(GOLDEN))
+    assert key in ref, "no stored oracle reference for %s: run tests/golden/make_golden.py" % key
+    return ref[key]
+
+
+def check_sampled_solution(x, ref, tol):
+    """The stored sample of the oracle's solution (>= 4096 entries on the full-size configs) against the
+    same entries of `x`: |x_S - want_S| <= tol |x_oracle| sqrt(|S| / n), the sampled form of rel-L2 <= tol
+    (no slack factor), and the norm of the whole vector."""
+    import numpy as np
+    idx = np.asarray(ref["sample_index"])
+    want = np.asarray(ref["sample_re"]) + 1j * np.asarray(ref["sample_im"])
+    got = x.ravel()[idx]
+    assert np.linalg.norm(got - want) <= tol * ref["x_norm"] * np.sqrt(len(idx) / x.size)
+    assert abs(np.linalg.norm(x.ravel()) - ref["x_norm"]) <= tol * ref["x_norm"]

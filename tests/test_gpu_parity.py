@@ -1,8 +1,6 @@
 """Parity of the CUDA path (through the C-ABI) with the CPU oracle, element by element on the
 same seeded inputs.  Tolerances are BASELINE.json north_star's: Dslash rel-L2 <= 1e-13 (fp64),
 CG solution rel <= 1e-9 at tol 1e-10 with iteration counts within +-2, tables bit-exact."""
-import json
-import os
 
 import numpy as np
 import pytest
@@ -10,10 +8,10 @@ import torch
 
 import oracle
 from paper_1311_2719_b200 import synth
+from lattice_util import check_sampled_solution, golden
 
 pytestmark = pytest.mark.gpu
 
-GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "oracle_cg_reference.json")
 DSLASH_TOL = 1e-13
 CG_TOL = 1e-9
 
@@ -240,24 +238,10 @@ def test_results_are_reproducible_run_to_run(lq):
 
 # ------------------------------------------------------------------ full-size configs
 
-def _golden(cfg):
-    if not os.path.exists(GOLDEN):
-        pytest.skip("tests/golden/oracle_cg_reference.json not generated")
-    ref = json.load(open(GOLDEN)).get("cfg%d" % cfg)
-    if ref is None:
-        pytest.skip("no stored oracle reference for cfg%d" % cfg)
-    return ref
-
-
-def _check_against_golden(c, u, b, x, it, res, ref):
+def _check_against_golden(c, x, it, res, ref):
     assert abs(it - ref["iters"]) <= 2
-    idx = np.asarray(ref["sample_index"])
-    want = np.asarray(ref["sample_re"]) + 1j * np.asarray(ref["sample_im"])
-    got = x.ravel()[idx]
-    # sampled entries of the oracle's solution; the norm of the whole oracle solution scales the error
-    assert np.linalg.norm(got - want) <= CG_TOL * ref["x_norm"] * np.sqrt(len(idx) / x.size) * 10
-    assert abs(np.linalg.norm(x.ravel()) - ref["x_norm"]) <= CG_TOL * ref["x_norm"]
-    assert res <= 2 * c["tol"]
+    check_sampled_solution(x, ref, CG_TOL)
+    assert res <= c["tol"] * (1 + 1e-6)      # the true residual itself meets the tolerance (not only the recursion's)
 
 
 def test_reconstruct_option_invalidates_loaded_gauge(lq):
@@ -277,26 +261,38 @@ def test_reconstruct_option_invalidates_loaded_gauge(lq):
 
 @pytest.mark.slow
 @pytest.mark.parametrize("recon", [18, 12])
-def test_cg_cfg3_bench_workload(lq, recon):
-    """32^4, m = 0.01 in the launch configuration bench.py times.  The oracle's own solve takes
-    minutes, so its iteration count and sampled solution entries are stored (make_golden.py);
-    the solution is also checked here with one oracle application of A (holds at any size)."""
-    c, u, b = synth.config_inputs(3)
+def test_cg_cfg3_bench_workload(lq, recon, cfg3_inputs, cfg3_oracle_cg):
+    """32^4, m = 0.01 in the launch configuration bench.py times, against the oracle's own CG on the same
+    inputs: the WHOLE solution vector at rel-L2 <= 1e-9, the iteration count within +-2,
+    and the stored oracle reference (tests/golden) which must agree with the oracle run of this session."""
+    c, u, b = cfg3_inputs
     with make_lattice(lq, c["dims"], 0, u, recon) as lat:
-        x, it, res, status = run_cg(lat, c, b, maxiter=50000)
-    assert status == 0 and res <= 2 * c["tol"]
+        lat.set_option(lq.OPT_CG_MODE, lq.CG_GRAPH)
+        lat.set_option(lq.OPT_CG_CHECK_EVERY, 8)
+        x, it, res, status = lat.cg_solve(c["param"], c["tol"], 50000, dev(b))
+        x = host(x)
+    want = cfg3_oracle_cg
+    assert status == 0 and want["status"] == 0
+    assert abs(it - want["iters"]) <= 2
+    assert rel(x, want["x"]) <= CG_TOL
+    assert abs(res - want["true_residual"]) <= 0.05 * want["true_residual"]
     ax = oracle.apply_MdagM(c["dims"], 0, u, c["param"], x)
     assert abs(rel(ax, b) - res) <= 1e-3 * res + 1e-13
-    _check_against_golden(c, u, b, x, it, res, _golden(3))
+    ref = golden("cfg3")
+    assert want["iters"] == ref["iters"]
+    check_sampled_solution(want["x"], ref, 1e-12)      # the stored sample is this oracle's solution
+    _check_against_golden(c, x, it, res, ref)
 
 
 @pytest.mark.slow
 def test_cg_cfg5(lq, cfg5_inputs):
+    """48^3 x 96, m = 0.005 (6 GB of links): iteration count (+-2) and 4096 sampled entries of the oracle's
+    solution from tests/golden (the oracle needs ten minutes for this solve), the true residual, and one
+    oracle application of A to the whole solution."""
     c, u, b = cfg5_inputs
     with make_lattice(lq, c["dims"], 0, u) as lat:
         x, it, res, status = run_cg(lat, c, b, maxiter=50000)
-    assert status == 0 and res <= 2 * c["tol"]
+    assert status == 0
     ax = oracle.apply_MdagM(c["dims"], 0, u, c["param"], x)
     assert abs(rel(ax, b) - res) <= 1e-3 * res + 1e-13
-    if os.path.exists(GOLDEN) and "cfg5" in json.load(open(GOLDEN)):
-        _check_against_golden(c, u, b, x, it, res, _golden(5))
+    _check_against_golden(c, x, it, res, golden("cfg5"))
