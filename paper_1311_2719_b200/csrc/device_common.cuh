@@ -98,11 +98,59 @@ __device__ __forceinline__ float2 ld_stream(const float2* p)
     asm volatile("ld.global.cs.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
     return v;
 }
+// Link loads by cache policy.  LP_STREAM: as above (fields larger than L2).  LP_L2: through L2 with normal
+// eviction and no L1 allocation -- for fields that FIT in L2 and are read by both parities of a full-lattice
+// operator (each link is the forward link of x and the backward link of x+mu^), so the second use and every
+// later iteration hits L2.  LP_L2_LAST: the same, marked evict-last.
+enum LinkPolicy { LP_STREAM = 0, LP_L2 = 1, LP_L2_LAST = 2, LP_DEFAULT = 3 };
+__device__ __forceinline__ unsigned long long l2_evict_last_policy()
+{
+    unsigned long long pol;
+    asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+template <int POLICY>
+__device__ __forceinline__ double2 ld_link(const double2* p)
+{
+    double2 v;
+    if (POLICY == LP_L2)
+        asm volatile("ld.global.cg.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
+    else if (POLICY == LP_L2_LAST)
+        asm volatile("ld.global.L1::no_allocate.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(l2_evict_last_policy()));
+    else if (POLICY == LP_DEFAULT)
+        asm volatile("ld.global.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
+    else
+        asm volatile("ld.global.cs.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
+    return v;
+}
+template <int POLICY>
+__device__ __forceinline__ float2 ld_link(const float2* p)
+{
+    float2 v;
+    if (POLICY == LP_L2)
+        asm volatile("ld.global.cg.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+    else if (POLICY == LP_L2_LAST)
+        asm volatile("ld.global.L1::no_allocate.L2::cache_hint.v2.f32 {%0, %1}, [%2], %3;" : "=f"(v.x), "=f"(v.y) : "l"(p), "l"(l2_evict_last_policy()));
+    else if (POLICY == LP_DEFAULT)
+        asm volatile("ld.global.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+    else
+        asm volatile("ld.global.cs.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+    return v;
+}
 // Vectors are re-read by up to 8 neighbouring sites: read-only path, keep in L1/L2.
 __device__ __forceinline__ double2 ld_keep(const double2* p) { return __ldg(p); }
 __device__ __forceinline__ float2 ld_keep(const float2* p) { return __ldg(p); }
 template <class C>
 __device__ __forceinline__ void st_vec(C* p, C v) { *p = v; }
+// x is read and written exactly once per CG iteration: stream it past the caches.
+__device__ __forceinline__ void st_stream(double2* p, double2 v)
+{
+    asm volatile("st.global.cs.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(v.x), "d"(v.y) : "memory");
+}
+__device__ __forceinline__ void st_stream(float2* p, float2 v)
+{
+    asm volatile("st.global.cs.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(v.x), "f"(v.y) : "memory");
+}
 
 // ------------------------------------------------------------------ complex helpers
 __device__ __forceinline__ double2 cmake(double re, double im) { return make_double2(re, im); }
@@ -166,12 +214,12 @@ __device__ __forceinline__ float2 to_cplx(double2 a, float2*) { return make_floa
 // RECON = 18: all nine entries.  RECON = 12: the first two rows; the third row of an SU(3) matrix
 // is the conjugated cross product of the first two ("two-column link compression",
 // SURVEY.md 8(f) row 1): 96 instead of 144 bytes per link from HBM for 42 extra flops.
-template <int RECON, class C>
+template <int RECON, class C, int POLICY = LP_STREAM>
 __device__ __forceinline__ void load_link(const C* __restrict__ p, size_t Vh, C U[9])
 {
     constexpr int NC = RECON / 2;
 #pragma unroll
-    for (int k = 0; k < NC; ++k) U[k] = ld_stream(p + k * Vh);
+    for (int k = 0; k < NC; ++k) U[k] = ld_link<POLICY>(p + k * Vh);
 }
 // Kept apart from load_link so that a hop can issue all its loads before the first dependent flop.
 template <int RECON, class C>

@@ -57,6 +57,7 @@ struct lqcd_ctx {
     int recon;  // 18 or 12 stored reals per link
     int congrad_precision;  // 64 or 32: which solver lqcd_congrad_host runs
     int f32_pairs;          // fp32 kernels of the mixed solver: two sites per thread with 128-bit loads
+    bool links_fit_l2;  // the stored link field is at most a third of the L2 (set by lqcd_load_gauge)
     bool wilson_eo;  // set while lqcd_wilson_solve_eo runs: the CG works on Mhat^+ Mhat, even half of the vectors
     // host side
     CgScalars* h_sc;  // pinned, 2 slots
@@ -251,17 +252,28 @@ WilsonArgs wilson_args(const lqcd_ctx* ctx, int parity, const cplx* in, cplx* ou
     return a;
 }
 
+template <int EPI, bool DAGGER, int LINKS>
+int launch_wilson_policy(lqcd_ctx* ctx, const WilsonArgs& a)
+{
+    // one-parity kernels: one block per tile of Vh; full-lattice kernels: tiles of the two parities alternate
+    const unsigned int tiles = blocks_for(ctx->g.Vh, kWilsonBlock);
+    const unsigned int grid = wilson_one_parity(EPI) ? tiles : 2 * tiles;
+    if (ctx->recon == 12)
+        wilson_dslash_kernel<EPI, DAGGER, kWilsonBlock, 12, LINKS><<<grid, kWilsonBlock, 0, ctx->stream>>>(a);
+    else
+        wilson_dslash_kernel<EPI, DAGGER, kWilsonBlock, 18, LINKS><<<grid, kWilsonBlock, 0, ctx->stream>>>(a);
+    LQCD_LAUNCH_CHECK();
+    return LQCD_OK;
+}
+
 template <int EPI, bool DAGGER>
 int launch_wilson(lqcd_ctx* ctx, const WilsonArgs& a)
 {
-    const size_t n = wilson_one_parity(EPI) ? (size_t)ctx->g.Vh : (size_t)ctx->g.V;
-    const unsigned int grid = blocks_for(n, kWilsonBlock);
-    if (ctx->recon == 12)
-        wilson_dslash_kernel<EPI, DAGGER, kWilsonBlock, 12><<<grid, kWilsonBlock, 0, ctx->stream>>>(a);
-    else
-        wilson_dslash_kernel<EPI, DAGGER, kWilsonBlock, 18><<<grid, kWilsonBlock, 0, ctx->stream>>>(a);
-    LQCD_LAUNCH_CHECK();
-    return LQCD_OK;
+    // Link cache policy (device_common.cuh): a full-lattice kernel uses every link twice within a short time
+    // (wilson_thread_site) -> through L2; a one-parity kernel uses every link once per launch -> streamed,
+    // unless the whole field stays in L2 from launch to launch (ctx->links_fit_l2).
+    if (!wilson_one_parity(EPI) || ctx->links_fit_l2) return launch_wilson_policy<EPI, DAGGER, LP_L2>(ctx, a);
+    return launch_wilson_policy<EPI, DAGGER, LP_STREAM>(ctx, a);
 }
 
 // ---------------------------------------------------------------- operator pieces
@@ -613,7 +625,7 @@ int lqcd_create(lqcd_ctx** out, int L0, int L1, int L2, int L3, int fermion_type
     c->g.V = V;
     c->g.Vh = (int)(V / 2);
     c->nvec = fermion_type == LQCD_STAGGERED ? 3 * (size_t)(V / 2) : 12 * (size_t)V;
-    c->max_blocks = (size_t)V / 64 + 4096;
+    c->max_blocks = (size_t)V / 32 + 4096;
     c->cg_mode = LQCD_CG_ASYNC;
     c->check_every = 4;
     c->recon = 18;
@@ -734,6 +746,12 @@ int lqcd_load_gauge(lqcd_ctx* ctx, const double* u_dev)
     LQCD_LAUNCH_CHECK();
     ctx->gauge_f_ready = false;
     ctx->gauge_loaded = true;
+    // B200: 126 MB of L2 in two partitions; data read by all SMs is cached in both, so about half of it is
+    // usable for a field every SM reads (75 MB of links at 16^3 x 32 were measured NOT to stay resident).
+    int dev = 0, l2 = 0;
+    LQCD_CUDA(cudaGetDevice(&dev));
+    LQCD_CUDA(cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev));
+    ctx->links_fit_l2 = V * 4 * (size_t)(ctx->recon / 2) * sizeof(cplx) <= (size_t)l2 / 3;
     return LQCD_OK;
 }
 

@@ -67,19 +67,10 @@ template <> struct GammaDR<3> { static constexpr int PI0 = 2, K0 = 0, PI1 = 3, K
 
 // One hop.  PLUS = false: projector (1 - gamma_mu); PLUS = true: (1 + gamma_mu).
 // ADJ = false: multiply by U (forward link at x); ADJ = true: by U^+ (link at x - mu^).
-template <int MU, bool PLUS, bool ADJ, int RECON>
-__device__ __forceinline__ void wilson_hop(const cplx* __restrict__ link, size_t Vh, const cplx* __restrict__ src,
-                                           size_t V, double sign, cplx acc[4][3])
+template <int MU, bool PLUS, bool ADJ>
+__device__ __forceinline__ void wilson_hop_math(const cplx U[9], const cplx psi[4][3], double sign, cplx acc[4][3])
 {
     typedef GammaDR<MU> G;
-    cplx U[9], psi[4][3];
-    load_link<RECON>(link, Vh, U);
-#pragma unroll
-    for (int s = 0; s < 4; ++s)
-#pragma unroll
-        for (int c = 0; c < 3; ++c) psi[s][c] = ld_keep(src + (size_t)(s * 3 + c) * V);
-    reconstruct_link<RECON>(U);
-
     // h_s = psi_s -+ i^K psi_pi(s)
     constexpr int KH0 = PLUS ? G::K0 : (G::K0 + 2) & 3;
     constexpr int KH1 = PLUS ? G::K1 : (G::K1 + 2) & 3;
@@ -112,7 +103,21 @@ __device__ __forceinline__ void wilson_hop(const cplx* __restrict__ link, size_t
     }
 }
 
-template <int MU, bool DAGGER, int RECON>
+template <int MU, bool PLUS, bool ADJ, int RECON, int LINKS>
+__device__ __forceinline__ void wilson_hop(const cplx* __restrict__ link, size_t Vh, const cplx* __restrict__ src,
+                                           size_t V, double sign, cplx acc[4][3])
+{
+    cplx U[9], psi[4][3];
+    load_link<RECON, cplx, LINKS>(link, Vh, U);
+#pragma unroll
+    for (int s = 0; s < 4; ++s)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) psi[s][c] = ld_keep(src + (size_t)(s * 3 + c) * V);
+    reconstruct_link<RECON>(U);
+    wilson_hop_math<MU, PLUS, ADJ>(U, psi, sign, acc);
+}
+
+template <int MU, bool DAGGER, int RECON, int LINKS>
 __device__ __forceinline__ void wilson_dir(const WilsonArgs& a, const Site& s, int parity, cplx acc[4][3])
 {
     const size_t Vh = (size_t)a.g.Vh, V = (size_t)a.g.V;
@@ -122,44 +127,35 @@ __device__ __forceinline__ void wilson_dir(const WilsonArgs& a, const Site& s, i
     const cplx* Uf = a.gauge + (size_t)((parity * 4 + MU) * (RECON / 2)) * Vh + s.e;
     const cplx* Ub = a.gauge + (size_t)(((1 - parity) * 4 + MU) * (RECON / 2)) * Vh + eb;
     // D: forward (1-gamma), backward (1+gamma);  D^+: forward (1+gamma), backward (1-gamma)
-    wilson_hop<MU, DAGGER, false, RECON>(Uf, Vh, a.in + other + ef, V, bc_fwd<MU>(a.g, s), acc);
-    wilson_hop<MU, !DAGGER, true, RECON>(Ub, Vh, a.in + other + eb, V, bc_bwd<MU>(a.g, s), acc);
+    wilson_hop<MU, DAGGER, false, RECON, LINKS>(Uf, Vh, a.in + other + ef, V, bc_fwd<MU>(a.g, s), acc);
+    wilson_hop<MU, !DAGGER, true, RECON, LINKS>(Ub, Vh, a.in + other + eb, V, bc_bwd<MU>(a.g, s), acc);
 }
 
-template <int EPI, bool DAGGER, int BLOCK, int RECON>
-__global__ void __launch_bounds__(BLOCK, LQCD_WILSON_MINB) wilson_dslash_kernel(const WilsonArgs a)
+// Which site a thread owns.  One-parity kernels cover the Vh sites of a.parity.  The full-lattice kernels
+// alternate the parities block by block (block 2k: tile k of the even sites, block 2k+1: tile k of the odd
+// sites), so that U_mu(x) is read as the forward link of x and as the backward link of x+mu^ within a short
+// time: with links loaded through L2 (LP_L2) the second use hits, and a full-lattice operator moves 576
+// instead of 1152 bytes of links per site from HBM (ncu at 16^3 x 32: 100.7 MB read by the M kernel =
+// 75.5 MB of links + 25.2 MB of p, against 160 MB with the parities one after the other and evict-first links).
+template <int EPI, int BLOCK>
+__device__ __forceinline__ bool wilson_thread_site(const WilsonArgs& a, int& parity, int& e)
 {
-    if (EPI == WE_M_NORM || EPI == WE_CGUPDATE || EPI == WE_EO_XPAY_NORM || EPI == WE_EO_CGUPDATE) {
-        if (a.sc->done) return;
-    }
-    const long long idx = (long long)blockIdx.x * BLOCK + threadIdx.x;
-    const size_t Vh = (size_t)a.g.Vh, V = (size_t)a.g.V;
-    bool active;
-    int parity, e;
     if (wilson_one_parity(EPI)) {
-        active = idx < (long long)Vh;
         parity = a.parity;
-        e = (int)idx;
+        e = blockIdx.x * BLOCK + threadIdx.x;
     } else {
-        active = idx < (long long)V;
-        parity = idx >= (long long)Vh ? 1 : 0;
-        e = (int)(idx - (long long)parity * (long long)Vh);
+        parity = blockIdx.x & 1;
+        e = (blockIdx.x >> 1) * BLOCK + threadIdx.x;
     }
-    const size_t gsite = (size_t)parity * Vh + (size_t)e;
+    return e < a.g.Vh;
+}
+__host__ __device__ constexpr bool wilson_full_lattice(int epi) { return !wilson_one_parity(epi); }
 
-    cplx acc[4][3];
-#pragma unroll
-    for (int s = 0; s < 4; ++s)
-#pragma unroll
-        for (int c = 0; c < 3; ++c) acc[s][c] = czero<cplx>();
-    if (active) {
-        const Site st = decode_site(a.g, parity, e);
-        wilson_dir<0, DAGGER, RECON>(a, st, parity, acc);
-        wilson_dir<1, DAGGER, RECON>(a, st, parity, acc);
-        wilson_dir<2, DAGGER, RECON>(a, st, parity, acc);
-        wilson_dir<3, DAGGER, RECON>(a, st, parity, acc);
-    }
-
+// Everything after the eight hops: the site-diagonal term, the fused CG updates and the grid-wide sums.
+template <int EPI, int BLOCK>
+__device__ __forceinline__ void wilson_epilogue(const WilsonArgs& a, bool active, size_t gsite, cplx acc[4][3])
+{
+    const size_t V = (size_t)a.g.V;
     if (EPI == WE_PLAIN) {
         if (active) {
 #pragma unroll
@@ -257,6 +253,34 @@ __global__ void __launch_bounds__(BLOCK, LQCD_WILSON_MINB) wilson_dslash_kernel(
     } else if (EPI == WE_RESIDUAL) {
         grid_sum<BLOCK>(local, a.rs, [sc](double res2) { sc->res2 = res2; });
     }
+}
+
+// LINKS: cache policy of the link loads (device_common.cuh).  Full-lattice kernels always LP_L2 (see
+// wilson_thread_site); one-parity kernels read every link once per launch: LP_STREAM unless the whole field is
+// small enough to stay in L2 from one launch to the next.
+template <int EPI, bool DAGGER, int BLOCK, int RECON, int LINKS>
+__global__ void __launch_bounds__(BLOCK, LQCD_WILSON_MINB) wilson_dslash_kernel(const WilsonArgs a)
+{
+    if (EPI == WE_M_NORM || EPI == WE_CGUPDATE || EPI == WE_EO_XPAY_NORM || EPI == WE_EO_CGUPDATE) {
+        if (a.sc->done) return;
+    }
+    int parity, e;
+    const bool active = wilson_thread_site<EPI, BLOCK>(a, parity, e);
+    const size_t gsite = (size_t)parity * (size_t)a.g.Vh + (size_t)e;
+
+    cplx acc[4][3];
+#pragma unroll
+    for (int s = 0; s < 4; ++s)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) acc[s][c] = czero<cplx>();
+    if (active) {
+        const Site st = decode_site(a.g, parity, e);
+        wilson_dir<0, DAGGER, RECON, LINKS>(a, st, parity, acc);
+        wilson_dir<1, DAGGER, RECON, LINKS>(a, st, parity, acc);
+        wilson_dir<2, DAGGER, RECON, LINKS>(a, st, parity, acc);
+        wilson_dir<3, DAGGER, RECON, LINKS>(a, st, parity, acc);
+    }
+    wilson_epilogue<EPI, BLOCK>(a, active, gsite, acc);
 }
 
 }  // namespace lqcd
