@@ -90,7 +90,21 @@ enum {
      * read them with 128-bit loads (lattices with L0 % 4 == 0; others use the one-site kernels).
      * 0: one site per thread.  The vectors are bit-identical either way; the partial sums are
      * grouped differently, so scalars differ in the last bits. */
-    LQCD_OPT_F32_PAIRS = 4
+    LQCD_OPT_F32_PAIRS = 4,
+    /* The iteration loop of lqcd_cg_solve as ONE cooperative kernel (staggered contexts; grid-wide barriers
+     * between the three phases of an iteration, no host round trip and no kernel boundary inside the loop:
+     * PAPER.md:100 "the entire conjugate gradient routine runs on the GPU").  -1 (default): automatic --
+     * used where the three-kernel iteration is bounded by its kernel boundaries, i.e. on lattices whose
+     * links fit the L2 cache (4^4, 16^4); 0: never; 1: always.  The iterates are bit-identical to the
+     * other modes run with 32-thread blocks (same arithmetic, same summation order: a warp of the
+     * cooperative kernel is one 32-thread block of the three-kernel path; 32 is what LQCD_OPT_STAG_BLOCK's
+     * automatic choice gives on those lattices); LQCD_OPT_CG_MODE / _CHECK_EVERY do not apply while it is
+     * in use (the exit test runs on the device every iteration). */
+    LQCD_OPT_PERSISTENT = 5,
+    /* Threads per block of the fp64 staggered kernels: 0 (default) = by lattice size (32 / 64 / 128: small
+     * lattices are latency-bound and gain from more, smaller blocks), or 32, 64, 128.  Changes how the
+     * per-block partial sums are grouped, hence the last bits of the inner products -- nothing else. */
+    LQCD_OPT_STAG_BLOCK = 6
 };
 
 /* Create a context for an L0 x L1 x L2 x L3 lattice (every extent even and >= 2; L = 2 is
@@ -140,6 +154,11 @@ int lqcd_apply_MdagM(lqcd_ctx *ctx, double mass_or_kappa, const double *in_dev, 
  * S1-S7 of SURVEY.md 8(a)): stops when <r,r> <= tol^2 <b,b> (tol = 0: run exactly maxiter
  * iterations) or after maxiter iterations (returns LQCD_MAXITER).  *iters = number of
  * applications of A inside the loop; *true_residual = |b - A x| / |b| from a fresh A.
+ * The status is decided by the RECURSION residual, as in the paper (betan.lt.delit):
+ * LQCD_OK means <r,r> of the iterated r met the rule; *true_residual is reported beside it and can
+ * exceed tol by rounding on ill-conditioned systems (32^4, m = 0.01: 9.94e-11 at tol 1e-10) -- a caller
+ * that needs the bound on the true residual compares *true_residual itself (the full-system, even-odd
+ * and slab solvers follow the same rule; lqcd_cg_solve_mixed decides on an fp64 true residual).
  * b = 0 gives x = 0, iters = 0, true_residual = 0.  b_dev and x_dev must not alias. */
 int lqcd_cg_solve(lqcd_ctx *ctx, double mass_or_kappa, double tol, int maxiter, const double *b_dev, double *x_dev,
                   int *iters, double *true_residual);

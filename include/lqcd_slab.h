@@ -38,6 +38,12 @@
  *     (B200_PROFILING.md: kernels that wait on one another must not share a GPU); with the slabs on
  *     several devices of one process (peer access enabled) it is a single-process multi-GPU solver.
  *
+ * VALIDATION STATUS: every call is parity-tested against the oracle of the undivided lattice with all
+ * slabs on ONE GPU (the *_group calls, and the nranks = 1 ring through the one-rank-per-process calls),
+ * where system-scope and device-scope fences behave alike.  The one-rank-per-process path with
+ * nranks > 1 (IPC-mapped mailboxes, peer stores over NVLink) has not yet run on more than one GPU:
+ * tests/test_gpu_slab.py holds a parity test that runs only where torch.cuda.device_count() >= 2.
+ *
  * Pointer suffixes, return codes, error text: as lqcd.h.  No CPU fallback.
  */
 #ifndef LQCD_SLAB_H
@@ -60,11 +66,14 @@ enum {
     LQCD_SLAB_OPT_GRAPH = 3,        /* 1 (default): when every slab of the call runs on one stream, each batch of
                                        CG iterations is replayed from one CUDA graph (an odd check_every is
                                        rounded up to even); 0: kernel-by-kernel launches.  Same iterates. */
-    LQCD_SLAB_OPT_FUSE_SYNC = 4     /* one-rank-per-process calls only.  1 (default): the last block of every kernel
-                                       that ends in a sum (the Dslash kernels of the CG, the p-update, the init)
-                                       also signals, waits and combines, so an iteration is three launches and
-                                       the exchange costs no kernel boundary; 0: a separate small launch per
-                                       synchronisation point, as the *_group calls always do.  Same iterates. */
+    LQCD_SLAB_OPT_FUSE_SYNC = 4     /* one-rank-per-process calls only.  1: the last block of every kernel that ends
+                                       in a sum (the Dslash kernels of the CG, the p-update, the init) also
+                                       signals, waits and combines, so an iteration is three launches and the
+                                       exchange costs no kernel boundary; 0: a separate small launch per
+                                       synchronisation point, as the *_group calls always do.  Same iterates.
+                                       Default: 1 for nranks = 1, 0 for nranks > 1 -- the fused tail has only
+                                       ever synchronised with itself (one GPU per box so far); switch it on
+                                       explicitly once the separate-launch form has run on real peers. */
 };
 
 /* Slab of rank `rank` of `nranks` for the global L0 x L1 x L2 x L3 staggered lattice.  L3/nranks must be

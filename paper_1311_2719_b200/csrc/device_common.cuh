@@ -140,6 +140,16 @@ __device__ __forceinline__ float2 ld_link(const float2* p)
 // Vectors are re-read by up to 8 neighbouring sites: read-only path, keep in L1/L2.
 __device__ __forceinline__ double2 ld_keep(const double2* p) { return __ldg(p); }
 __device__ __forceinline__ float2 ld_keep(const float2* p) { return __ldg(p); }
+// Vector loads by coherence need.  VL_NC: the read-only (non-coherent) path -- only for data no block of the
+// running kernel writes.  VL_PLAIN: ordinary L1-allocating loads, for kernels that read what other blocks of
+// the SAME launch wrote before a grid-wide barrier (cg_persistent.cuh; the barrier's fences invalidate L1).
+enum VecLoad { VL_NC = 0, VL_PLAIN = 1 };
+template <int VL, class C>
+__device__ __forceinline__ C ld_vec(const C* p)
+{
+    if (VL == VL_PLAIN) return *p;
+    return __ldg(p);
+}
 template <class C>
 __device__ __forceinline__ void st_vec(C* p, C v) { *p = v; }
 // x is read and written exactly once per CG iteration: stream it past the caches.

@@ -11,6 +11,7 @@
 
 #include "../../include/lqcd.h"
 #include "cg_kernels.cuh"
+#include "cg_persistent.cuh"
 #include "stag_dslash.cuh"
 #include "stag_dslash_f32x2.cuh"
 #include "wilson_dslash.cuh"
@@ -57,6 +58,8 @@ struct lqcd_ctx {
     int recon;  // 18 or 12 stored reals per link
     int congrad_precision;  // 64 or 32: which solver lqcd_congrad_host runs
     int f32_pairs;          // fp32 kernels of the mixed solver: two sites per thread with 128-bit loads
+    int stag_block;         // 0 auto (stag_block_for), or 32 / 64 / 128 threads per block of the fp64 staggered kernels
+    int persistent;         // -1 auto, 0 never, 1 always: the CG loop as one cooperative kernel (cg_persistent.cuh)
     bool links_fit_l2;  // the stored link field is at most a third of the L2 (set by lqcd_load_gauge)
     bool wilson_eo;  // set while lqcd_wilson_solve_eo runs: the CG works on Mhat^+ Mhat, even half of the vectors
     // host side
@@ -171,6 +174,7 @@ StagArgsD stag_args(const lqcd_ctx* ctx, int parity, const cplx* in, cplx* out)
 // 32^4 234.9, 242.6, 267.3 per iteration: profiles/r01_bench.md).
 int stag_block_for(const lqcd_ctx* ctx)
 {
+    if (ctx->stag_block) return ctx->stag_block;  // LQCD_OPT_STAG_BLOCK
     const long long blocks128 = ((long long)ctx->g.Vh + 127) / 128;
     if (blocks128 < 2 * 148) return 32;
     if (blocks128 < 8 * 148) return 64;
@@ -383,6 +387,59 @@ int ensure_host(lqcd_ctx* ctx)
     return LQCD_OK;
 }
 
+// ---------------------------------------------------------------- the loop as one cooperative kernel
+// Used for the fp64 staggered CG where an iteration is bounded by its kernel boundaries: the links fit the
+// L2 (ctx->links_fit_l2), so the three kernels of an iteration take a few microseconds each.
+bool use_persistent(const lqcd_ctx* ctx)
+{
+    if (ctx->fermion != LQCD_STAGGERED || ctx->wilson_eo) return false;
+    if (ctx->persistent >= 0) return ctx->persistent == 1;
+    return ctx->links_fit_l2;
+}
+
+template <int RECON>
+int launch_persistent_recon(lqcd_ctx* ctx, double mass, cplx* x, int niter)
+{
+    PersistArgs a;
+    memset(&a, 0, sizeof a);
+    a.g = ctx->g;
+    a.gauge = ctx->gauge();
+    a.p = ctx->p();
+    a.t = ctx->t();
+    a.x = x;
+    a.r = ctx->r();
+    a.m2 = mass * mass;
+    a.sc = ctx->sc();
+    a.hist = ctx->hist();
+    a.partials = ctx->rs().partials;
+    a.bar = ctx->rs().ticket + 16;  // the 256-byte ticket area: word 0 = reduction ticket, word 16 = grid barrier
+    a.nvb = (int)blocks_for(ctx->g.Vh, 32);
+    a.vgrid = (int)vec_grid(ctx);
+    a.niter = niter;
+    if ((size_t)(2 * a.nvb + a.vgrid) > ctx->max_blocks) return fail(ctx, LQCD_ENOMEM, "partial-sum area too small for the persistent kernel");
+    int dev = 0, nsm = 0, per_sm = 0, coop = 0;
+    LQCD_CUDA(cudaGetDevice(&dev));
+    LQCD_CUDA(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
+    if (!coop) return fail(ctx, LQCD_ECUDA, "device does not support cooperative launches");
+    LQCD_CUDA(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+    LQCD_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, stag_cg_persistent_kernel<RECON>, kPersistBlock, 0));
+    if (per_sm < 1) return fail(ctx, LQCD_ECUDA, "persistent CG kernel does not fit an SM");
+    // one block per SM at most, eight virtual blocks (warps) per block at a time
+    long long grid = (a.nvb + kPersistBlock / 32 - 1) / (kPersistBlock / 32);
+    if (grid > nsm) grid = nsm;
+    LQCD_CUDA(cudaMemsetAsync(a.bar, 0, sizeof(unsigned int), ctx->stream));
+    void* params[] = { (void*)&a };
+    LQCD_CUDA(cudaLaunchCooperativeKernel((const void*)stag_cg_persistent_kernel<RECON>, dim3((unsigned int)grid), dim3(kPersistBlock),
+                                          params, 0, ctx->stream));
+    ctx->launches++;
+    return LQCD_OK;
+}
+
+int launch_persistent(lqcd_ctx* ctx, double mass, cplx* x, int niter)
+{
+    return ctx->recon == 12 ? launch_persistent_recon<12>(ctx, mass, x, niter) : launch_persistent_recon<18>(ctx, mass, x, niter);
+}
+
 // Init (S6) and the iteration loop (S1-S5) of the conjugate gradient on A x = b.  On return the
 // stream is idle and ctx->h_sc[0] holds the final scalars (iter, rr_new, thresh, bb).
 int cg_run(lqcd_ctx* ctx, double mass_or_kappa, double tol, int maxiter, const cplx* b, cplx* x)
@@ -394,7 +451,16 @@ int cg_run(lqcd_ctx* ctx, double mass_or_kappa, double tol, int maxiter, const c
     LQCD_LAUNCH_CHECK();
 
     CgScalars* h = ctx->h_sc;
-    if (ctx->cg_mode == LQCD_CG_SYNC) {
+    if (use_persistent(ctx)) {
+        // one launch runs the loop to the exit rule (or maxiter); the scalars come back once
+        if (maxiter > 0) {
+            rc = launch_persistent(ctx, mass_or_kappa, x, maxiter);
+            if (rc) return rc;
+        }
+        rc = read_scalars(ctx, 0);
+        if (rc) return rc;
+        LQCD_CUDA(cudaEventSynchronize(ctx->ev[0]));
+    } else if (ctx->cg_mode == LQCD_CG_SYNC) {
         // The paper's loop: one scalar comes back per iteration, the exit test runs on the host
         // (PAPER.md:75-76, :91-93, :100).
         rc = read_scalars(ctx, 0);
@@ -631,6 +697,7 @@ int lqcd_create(lqcd_ctx** out, int L0, int L1, int L2, int L3, int fermion_type
     c->recon = 18;
     c->congrad_precision = 64;
     c->f32_pairs = 1;
+    c->persistent = -1;
 
     size_t off = 0;
     const size_t vec_bytes = align_up(c->nvec * sizeof(cplx));
@@ -725,6 +792,16 @@ int lqcd_set_option(lqcd_ctx* ctx, int option, int value)
     if (option == LQCD_OPT_F32_PAIRS) {
         if (value != 0 && value != 1) return fail(ctx, LQCD_EARG, "f32_pairs must be 0 or 1");
         ctx->f32_pairs = value;
+        return LQCD_OK;
+    }
+    if (option == LQCD_OPT_STAG_BLOCK) {
+        if (value != 0 && value != 32 && value != 64 && value != 128) return fail(ctx, LQCD_EARG, "stag_block must be 0 (auto), 32, 64 or 128");
+        ctx->stag_block = value;
+        return LQCD_OK;
+    }
+    if (option == LQCD_OPT_PERSISTENT) {
+        if (value < -1 || value > 1) return fail(ctx, LQCD_EARG, "persistent must be -1 (auto), 0 or 1");
+        ctx->persistent = value;
         return LQCD_OK;
     }
     return fail(ctx, LQCD_EARG, "unknown option %d", option);

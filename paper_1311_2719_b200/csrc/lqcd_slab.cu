@@ -620,7 +620,7 @@ int lqcd_slab_create(lqcd_slab** out, int L0, int L1, int L2, int L3, int rank, 
     c->check_every = 8;
     c->timeout_ms = 20000;
     c->use_graph = 1;
-    c->fuse_sync = 1;
+    c->fuse_sync = nranks == 1 ? 1 : 0;  // see LQCD_SLAB_OPT_FUSE_SYNC: unvalidated across GPUs
 
     size_t off = 0;
     const size_t vec_bytes = align_up(c->nvec * sizeof(cplx));

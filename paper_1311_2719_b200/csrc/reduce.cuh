@@ -156,11 +156,7 @@ __device__ __forceinline__ void grid_sum_block(double local, bool wrote_peer, co
     double s = block_sum<BLOCK>(local);
     if (threadIdx.x == 0) {
         rs.partials[blockIdx.x] = s;
-#if defined(LQCD_SLAB_FENCE_EXPERIMENT) && (LQCD_SLAB_FENCE_EXPERIMENT & 4)
-        if (false)
-#else
         if (any_peer)
-#endif
             __threadfence_system();
         else
             __threadfence();

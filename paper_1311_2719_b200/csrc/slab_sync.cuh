@@ -4,19 +4,6 @@
 #pragma once
 #include "reduce.cuh"
 
-// System-scope fences of the protocol.  LQCD_SLAB_FENCE_EXPERIMENT (a bit mask, measurement only, never
-// set in a build that talks to another GPU) narrows fence i to device scope to time what each one costs.
-#ifndef LQCD_SLAB_FENCE_EXPERIMENT
-#define LQCD_SLAB_FENCE_EXPERIMENT 0
-#endif
-#define LQCD_SLAB_FENCE(bit)                                   \
-    do {                                                       \
-        if (LQCD_SLAB_FENCE_EXPERIMENT & (bit))                \
-            __threadfence();                                   \
-        else                                                   \
-            __threadfence_system();                            \
-    } while (0)
-
 namespace lqcd {
 
 constexpr int kSlabMaxRanks = 16;
@@ -68,7 +55,7 @@ __device__ __forceinline__ void slab_signal(const SlabSyncArgs& a, unsigned long
 {
     double* dst = a.peer_slot[r] + ((seq & 1ull) * a.nranks + a.rank) * 2;
     for (int k = 0; k < a.nvals; ++k) dst[k] = a.ss->part[k];
-    LQCD_SLAB_FENCE(1);
+    __threadfence_system();  // release: slots (and the producer's face stores) before the flag
     *(volatile unsigned long long*)(a.peer_flag[r] + a.rank) = seq;
 }
 
@@ -101,7 +88,7 @@ __device__ __forceinline__ void slab_combine(const SlabSyncArgs& a, unsigned lon
         a.sc->done = 1;
         return;
     }
-    LQCD_SLAB_FENCE(2);
+    __threadfence_system();  // acquire: the flags before the slots and the ghost faces
     double total[2] = { 0.0, 0.0 };
     const volatile double* s = a.own.slot + (seq & 1ull) * a.nranks * 2;
     for (int q = 0; q < a.nranks; ++q)

@@ -70,7 +70,7 @@ struct StagArgs {
     SlabArgs<C> sl;  // used by the SLAB instantiations only
 };
 
-template <int MU, int RECON, bool SLAB, class C>
+template <int MU, int RECON, bool SLAB, class C, int VL = VL_NC>
 __device__ __forceinline__ void stag_hop(const StagArgs<C>& a, const Site& s, C acc[3])
 {
     constexpr int NC = RECON / 2;
@@ -108,10 +108,10 @@ __device__ __forceinline__ void stag_hop(const StagArgs<C>& a, const Site& s, C 
         const C* Ub = a.gauge + (size_t)(((1 - a.parity) * 4 + MU) * NC) * Vh + eb;
         load_link<RECON>(Uf, Vh, U);
 #pragma unroll
-        for (int c = 0; c < 3; ++c) vf[c] = ld_keep(a.in + c * Vh + ef);
+        for (int c = 0; c < 3; ++c) vf[c] = ld_vec<VL>(a.in + c * Vh + ef);
         load_link<RECON>(Ub, Vh, W);
 #pragma unroll
-        for (int c = 0; c < 3; ++c) vb[c] = ld_keep(a.in + c * Vh + eb);
+        for (int c = 0; c < 3; ++c) vb[c] = ld_vec<VL>(a.in + c * Vh + eb);
         sf = eta * bc_fwd<MU>(a.g, s);
         sb = -eta * bc_bwd<MU>(a.g, s);
     }

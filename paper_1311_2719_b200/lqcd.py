@@ -20,7 +20,7 @@ STAGGERED, WILSON = 0, 1
 EVEN, ODD = 0, 1
 OK, MAXITER = 0, 1
 CG_SYNC, CG_ASYNC, CG_GRAPH = 0, 1, 2
-OPT_CG_MODE, OPT_CG_CHECK_EVERY, OPT_RECONSTRUCT, OPT_CONGRAD_PRECISION, OPT_F32_PAIRS = 0, 1, 2, 3, 4
+OPT_CG_MODE, OPT_CG_CHECK_EVERY, OPT_RECONSTRUCT, OPT_CONGRAD_PRECISION, OPT_F32_PAIRS, OPT_PERSISTENT, OPT_STAG_BLOCK = 0, 1, 2, 3, 4, 5, 6
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _ROOT = os.path.dirname(_HERE)

@@ -168,6 +168,7 @@ def test_cg_matches_oracle(lq, cfg, recon):
 def test_cg_modes_give_identical_iterates(lq):
     c, u, b = synth.config_inputs(1)
     with make_lattice(lq, c["dims"], 0, u) as lat:
+        lat.set_option(lq.OPT_PERSISTENT, 0)      # the three-kernel solver and its host loops (auto would pick the one-kernel loop)
         x0, it0, res0, _ = run_cg(lat, c, b, mode=lq.CG_SYNC)
         h0 = lat.cg_history().numpy()
         for every in (1, 3, 16):
@@ -179,6 +180,39 @@ def test_cg_modes_give_identical_iterates(lq):
         assert it2 == it0 and res2 == res0 and np.array_equal(x0, x2)
 
 
+@pytest.mark.parametrize("dims,recon,every", [((4, 4, 4, 4), 18, 8), ((16, 16, 16, 16), 18, 8), ((16, 16, 16, 16), 12, 3),
+                                              ((10, 6, 6, 4), 18, 8), ((6, 4, 2, 2), 12, 1), ((2, 2, 2, 2), 18, 8),
+                                              ((24, 24, 24, 16), 18, 8)])
+def test_cg_persistent_kernel_changes_no_bit(lq, dims, recon, every):
+    """The iteration loop as one cooperative kernel (LQCD_OPT_PERSISTENT, cg_persistent.cuh) against the
+    three-kernel solver: same arithmetic, same summation order, so solution, iteration count, residual
+    history and true residual are bit-identical -- in one physical block (2^4, 4^4: no grid barrier), on
+    ragged tiles, with more virtual blocks than resident warps (24^3 x 16: 3456 on 148 x 8), both link
+    storages; and both agree with the oracle."""
+    mass = 0.05
+    u = synth.gauge_field(dims, "haar", 31)
+    b = synth.source(dims, "staggered", 32)
+    got = {}
+    with make_lattice(lq, dims, 0, u, recon) as lat:
+        lat.set_option(lq.OPT_CG_MODE, lq.CG_GRAPH)
+        lat.set_option(lq.OPT_CG_CHECK_EVERY, every)
+        lat.set_option(lq.OPT_STAG_BLOCK, 32)         # a warp of the one-kernel loop = one 32-thread block of the three-kernel path
+        for pers in (0, 1):
+            lat.set_option(lq.OPT_PERSISTENT, pers)
+            n0 = lat.kernel_launches()
+            x, it, res, status = lat.cg_solve(mass, 1e-10, 20000, dev(b))
+            got[pers] = (host(x), it, res, status, lat.cg_history().numpy(), lat.kernel_launches() - n0)
+            xk, itk, _, stk = lat.cg_solve(mass, 0.0, 7, dev(b))                   # tol = 0: exactly 7 iterations
+            got[pers] += (host(xk), itk, stk)
+    a, p = got[0], got[1]
+    assert p[5] == 4 and a[5] > 3 * a[1]              # init + ONE loop kernel + the two kernels of the final check
+    assert a[1] == p[1] and a[2] == p[2] and a[3] == p[3] == 0
+    assert np.array_equal(a[0], p[0]) and np.array_equal(a[4], p[4])
+    assert a[7] == p[7] == 7 and a[8] == p[8] == 1 and np.array_equal(a[6], p[6])
+    want = oracle.cg(dims, 0, u, mass, 1e-10, 20000, b)
+    assert abs(p[1] - want["iters"]) <= 2 and rel(p[0], want["x"]) <= CG_TOL
+
+
 @pytest.mark.parametrize("mode", [0, 1, 2])
 def test_cg_fixed_iteration_count_matches_oracle_iterate(lq, mode):
     """tol = 0 runs exactly maxiter iterations: compare the iterate x_k itself."""
@@ -186,6 +220,7 @@ def test_cg_fixed_iteration_count_matches_oracle_iterate(lq, mode):
     for k in (1, 5, 17):
         want = oracle.cg(c["dims"], 0, u, c["param"], 0.0, k, b)
         with make_lattice(lq, c["dims"], 0, u) as lat:
+            lat.set_option(lq.OPT_PERSISTENT, 0)
             x, it, res, status = run_cg(lat, c, b, mode=mode, maxiter=k, tol=0.0)
         assert status == 1 and it == k == want["iters"]
         assert rel(x, want["x"]) <= 1e-12
@@ -195,7 +230,8 @@ def test_cg_fixed_iteration_count_matches_oracle_iterate(lq, mode):
 def test_cg_edge_cases(lq):
     c, u, b = synth.config_inputs(1)
     with make_lattice(lq, c["dims"], 0, u) as lat:
-        for mode in (lq.CG_SYNC, lq.CG_ASYNC, lq.CG_GRAPH):
+        for mode, pers in ((lq.CG_SYNC, 0), (lq.CG_ASYNC, 0), (lq.CG_GRAPH, 0), (lq.CG_GRAPH, 1)):
+            lat.set_option(lq.OPT_PERSISTENT, pers)
             x, it, res, status = run_cg(lat, c, np.zeros_like(b), mode=mode)
             assert it == 0 and res == 0.0 and status == 0 and not x.any()          # b = 0
             x, it, res, status = run_cg(lat, c, b, mode=mode, maxiter=0)

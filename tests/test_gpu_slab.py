@@ -389,3 +389,81 @@ def test_slab_ipc_mailboxes_between_two_processes():
     for p in procs:
         p.join(timeout=120)
     assert all(g["ok"] for g in got), got
+
+
+# ------------------------------------------------------------------ two GPUs, one process each (runs only where two are visible)
+def _two_gpu_worker(rank, world, port, fuse, out):
+    """One rank per process and per GPU: IPC-mapped mailboxes, face stores and flags over NVLink, compute calls on
+    both sides -- the configuration a one-GPU box cannot run (two kernels that wait on one another must not
+    share a GPU).  Each rank reports its slab of D b, A b and the CG solution; the parent compares the
+    assembled vectors with the oracle of the undivided lattice."""
+    import os
+    import sys
+    os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+    import torch
+    import torch.distributed as dist
+    from paper_1311_2719_b200 import slab as sl, synth
+    res, msg = None, ""
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        dims, mass = (8, 8, 8, 8), 0.1
+        dev = torch.device("cuda", rank)
+        torch.cuda.set_device(dev)
+        u = torch.from_numpy(synth.gauge_field(dims, "haar", 7))
+        b = torch.from_numpy(synth.source(dims, "staggered", 8))
+        s = sl.Slab(dims, rank, world, device=dev)
+        s.set_option(sl.OPT_TIMEOUT_MS, 5000)
+        s.set_option(sl.OPT_FUSE_SYNC, fuse)
+        s.connect_ipc()
+        ul = sl.local_gauge(u, dims, rank, world)
+        ub = sl.exchange_u3_below(ul, dims, rank, world)      # the set-up exchange over torch.distributed
+        s.load_gauge(ul.to(dev), ub.to(dev))
+        bl = sl.local_vector(b, dims, rank, world).to(dev)
+        d, a, x = s.new_vector(), s.new_vector(), s.new_vector()
+        s.dslash(1, bl, d)
+        s.apply_MdagM(mass, bl, a)
+        _, it, tr, st = s.cg_solve(mass, 1e-10, 5000, bl, x)
+        s.stream.synchronize()
+        res = dict(d=d.cpu().numpy(), a=a.cpu().numpy(), x=x.cpu().numpy(), iters=it, true_residual=tr, status=st,
+                   sync_points=s.sync_points())
+        dist.barrier()
+        s.close()
+    except Exception as e:  # pragma: no cover - reported through the queue
+        msg = repr(e)
+    out.put(dict(rank=rank, res=res, msg=msg))
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("fuse", [0, 1])
+def test_slab_two_gpus_one_process_each(fuse):
+    import socket
+    import torch.multiprocessing as mp
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs: kernels of two ranks that wait on one another must not share a device")
+    import oracle
+    from paper_1311_2719_b200 import synth
+    sock = socket.socket()
+    sock.bind(("127.0.0.1", 0))
+    port = sock.getsockname()[1]
+    sock.close()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_two_gpu_worker, args=(i, 2, port, fuse, q)) for i in range(2)]
+    for p in procs:
+        p.start()
+    got = sorted((q.get(timeout=600) for _ in procs), key=lambda g: g["rank"])
+    for p in procs:
+        p.join(timeout=120)
+    assert all(g["res"] is not None for g in got), [g["msg"] for g in got]
+    dims, mass = (8, 8, 8, 8), 0.1
+    u = synth.gauge_field(dims, "haar", 7)
+    b = synth.source(dims, "staggered", 8)
+    cat = lambda k: np.concatenate([g["res"][k] for g in got], axis=1)
+    assert rel(cat("d"), oracle.dslash(dims, 0, u, 1, b)) <= 1e-13
+    assert rel(cat("a"), oracle.apply_MdagM(dims, 0, u, mass, b)) <= 1e-13
+    want = oracle.cg(dims, 0, u, mass, 1e-10, 5000, b)
+    assert got[0]["res"]["iters"] == got[1]["res"]["iters"] and abs(got[0]["res"]["iters"] - want["iters"]) <= 2
+    assert got[0]["res"]["true_residual"] == got[1]["res"]["true_residual"]      # rank-ordered sums: bit-identical scalars
+    assert all(g["res"]["status"] == 0 for g in got)
+    assert rel(cat("x"), want["x"]) <= 1e-9
