@@ -50,6 +50,7 @@ __global__ void __launch_bounds__(BLOCK) cg_init_kernel(const cplx* __restrict__
         sc->done = (bb == 0.0 || maxiter <= 0) ? 1 : 0;  // b = 0: x = 0, iters = 0 (reading A11)
         sc->pause = 0;
         sc->nupd = 0;
+        sc->xdue = 0;
         hist[0] = bb;
     });
 }
@@ -144,6 +145,39 @@ __global__ void __launch_bounds__(BLOCK) cg_pupdate_kernel(const C* __restrict__
         local += cnorm2(ps);
     }
     grid_sum<BLOCK>(local, rs, [sc](double pp) { sc->pp = pp; });
+}
+
+// The vector kernel of a Wilson CG iteration: x += alpha p (the second half of S3, moved here
+// because this kernel reads p anyway -- the Dslash kernel that updates r then never touches p or x), then S5:
+// p = r + beta p, pp = <p,p> unless the exit rule has fired.  `xdue` makes a pre-enqueued launch after
+// convergence a no-op without losing the x update of the converging iteration.
+template <int BLOCK>
+__global__ void __launch_bounds__(BLOCK) cg_xpupdate_kernel(const cplx* __restrict__ r, cplx* __restrict__ p, cplx* __restrict__ x,
+                                                            VecLayout lay, CgScalars* sc, ReduceScratch rs)
+{
+    if (!sc->xdue) return;
+    const double alpha = sc->alpha, beta = sc->beta;
+    const bool done = sc->done != 0;
+    double local = 0.0;
+    for (size_t j = (size_t)blockIdx.x * BLOCK + threadIdx.x; j < lay.n; j += (size_t)gridDim.x * BLOCK) {
+        const size_t i = lay.at(j);
+        double2 pv = p[i];
+        double2 xv = x[i];
+        xv.x = fma(alpha, pv.x, xv.x);   // x = x + alpha p
+        xv.y = fma(alpha, pv.y, xv.y);
+        st_stream(x + i, xv);
+        if (!done) {
+            const double2 rv = r[i];
+            pv.x = fma(beta, pv.x, rv.x);
+            pv.y = fma(beta, pv.y, rv.y);
+            p[i] = pv;
+            local += cnorm2(pv);
+        }
+    }
+    grid_sum<BLOCK>(local, rs, [sc, done](double pp) {
+        if (!done) sc->pp = pp;
+        sc->xdue = 0;
+    });
 }
 
 // S0: canonical u[g][mu][3][3] (array of structures, 576 B per site, fp64) ->

@@ -152,6 +152,8 @@ __device__ __forceinline__ C ld_vec(const C* p)
 }
 template <class C>
 __device__ __forceinline__ void st_vec(C* p, C v) { *p = v; }
+// Ask L2 for the 128-byte line of p; nothing is returned and no register waits for it.
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 // x is read and written exactly once per CG iteration: stream it past the caches.
 __device__ __forceinline__ void st_stream(double2* p, double2 v)
 {

@@ -341,10 +341,14 @@ int cg_iteration_kernels(lqcd_ctx* ctx, double param, cplx* x)
     return launch_wilson<WE_CGUPDATE, true>(ctx, a);
 }
 
-int cg_pupdate(lqcd_ctx* ctx)  // S5
+int cg_pupdate(lqcd_ctx* ctx, cplx* x)  // S5 (Wilson: preceded by the x += alpha p of S3, see cg_xpupdate_kernel)
 {
-    cg_pupdate_kernel<kVecBlock, cplx><<<vec_grid(ctx), kVecBlock, 0, ctx->stream>>>(ctx->r(), ctx->p(), vec_layout(ctx), ctx->sc(),
-                                                                              ctx->rs());
+    if (ctx->fermion == LQCD_WILSON)
+        cg_xpupdate_kernel<kVecBlock><<<vec_grid(ctx), kVecBlock, 0, ctx->stream>>>(ctx->r(), ctx->p(), x, vec_layout(ctx), ctx->sc(),
+                                                                                 ctx->rs());
+    else
+        cg_pupdate_kernel<kVecBlock, cplx><<<vec_grid(ctx), kVecBlock, 0, ctx->stream>>>(ctx->r(), ctx->p(), vec_layout(ctx), ctx->sc(),
+                                                                                  ctx->rs());
     LQCD_LAUNCH_CHECK();
     return LQCD_OK;
 }
@@ -354,7 +358,7 @@ int enqueue_batch(lqcd_ctx* ctx, double param, cplx* x, int batch)
     for (int k = 0; k < batch; ++k) {
         int rc = cg_iteration_kernels(ctx, param, x);
         if (rc) return rc;
-        rc = cg_pupdate(ctx);
+        rc = cg_pupdate(ctx, x);
         if (rc) return rc;
     }
     return LQCD_OK;
@@ -472,9 +476,10 @@ int cg_run(lqcd_ctx* ctx, double mass_or_kappa, double tol, int maxiter, const c
             rc = read_scalars(ctx, 0);
             if (rc) return rc;
             LQCD_CUDA(cudaEventSynchronize(ctx->ev[0]));
-            if (h[0].done) break;
-            rc = cg_pupdate(ctx);
+            if (h[0].done && ctx->fermion != LQCD_WILSON) break;
+            rc = cg_pupdate(ctx, x);  // Wilson: also after the exit rule has fired -- the kernel holds the last x += alpha p
             if (rc) return rc;
+            if (h[0].done) break;
         }
     } else {
         // Same kernels, same order; batches of `check_every` iterations are enqueued while the

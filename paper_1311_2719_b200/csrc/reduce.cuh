@@ -32,7 +32,9 @@ struct CgScalars {
     int pause;        // mixed precision: 1 = a reliable update is due; the fp32 iteration kernels are
                       // no-ops until the update sequence has run (it clears the flag)
     int nupd;         // mixed precision: reliable updates completed
-    int pad[3];
+    int xdue;         // Wilson solvers: 1 = the x += alpha p of the last iteration is still to be done by the
+                      // vector kernel that follows the update of r (cg_xpupdate_kernel clears it)
+    int pad[2];
 };
 static_assert(sizeof(CgScalars) == 128, "CgScalars is copied to the host as one 128-byte block");
 

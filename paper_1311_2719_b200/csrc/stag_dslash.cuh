@@ -284,11 +284,21 @@ __device__ __forceinline__ void stag_dslash_body(const StagArgs<C>& a, const Sla
         double local = 0.0;
         if (active) {
             const double alpha = a.sc->alpha;
+            // all nine operands are loaded before the first store: p, x and r may alias as far as the compiler
+            // can tell, so a load placed after a store waits for it (three serial round trips, colour by colour)
+            C p3[3], x3[3], r3[3];
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
                 const size_t i = c * Vh + e;
-                const double2 pv = to_d(a.p[i]), q = to_d(acc[c]);
-                double2 xv = to_d(a.x[i]), rv = to_d(a.r[i]);
+                p3[c] = a.p[i];
+                x3[c] = a.x[i];
+                r3[c] = a.r[i];
+            }
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const size_t i = c * Vh + e;
+                const double2 pv = to_d(p3[c]), q = to_d(acc[c]);
+                double2 xv = to_d(x3[c]), rv = to_d(r3[c]);
                 const double2 ap = cmake(fma(a.m2, pv.x, -q.x), fma(a.m2, pv.y, -q.y));
                 xv.x = fma(alpha, pv.x, xv.x);   // x = x + alpha p
                 xv.y = fma(alpha, pv.y, xv.y);

@@ -140,13 +140,22 @@ __global__ void __launch_bounds__(BLOCK, LQCD_STAG_MINB_F32X2) stag_dslash_f32x2
     } else {
         if (active) {
             const double alpha = a.sc->alpha;
+            // all operands loaded before the first store (see SE_CGUPDATE in stag_dslash.cuh)
+            float4 pq[3], xq[3], rq[3];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const size_t i = c * Vh + e;
+                pq[c] = *(const float4*)(a.p + i);
+                xq[c] = *(const float4*)(a.x + i);
+                rq[c] = *(const float4*)(a.r + i);
+            }
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
                 const size_t i = c * Vh + e;
                 cplxf p2[2], x2[2], r2[2];
-                split(*(const float4*)(a.p + i), p2[0], p2[1]);
-                split(*(const float4*)(a.x + i), x2[0], x2[1]);
-                split(*(const float4*)(a.r + i), r2[0], r2[1]);
+                split(pq[c], p2[0], p2[1]);
+                split(xq[c], x2[0], x2[1]);
+                split(rq[c], r2[0], r2[1]);
 #pragma unroll
                 for (int k = 0; k < 2; ++k) {
                     const double2 pv = to_d(p2[k]), q = to_d(acc[k][c]);

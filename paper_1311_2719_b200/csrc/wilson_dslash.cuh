@@ -21,6 +21,17 @@
 #ifndef LQCD_WILSON_MINB
 #define LQCD_WILSON_MINB 4
 #endif
+// Components per batch of the epilogue's loads (all loads of a batch precede its first store): one vector
+// (M, M + norm) and two vectors (the update of r) per component.
+#ifndef LQCD_WILSON_EPI_BATCH_M
+#define LQCD_WILSON_EPI_BATCH_M 6
+#endif
+#ifndef LQCD_WILSON_EPI_BATCH_U
+#define LQCD_WILSON_EPI_BATCH_U 6
+#endif
+#ifndef LQCD_WILSON_PREFETCH
+#define LQCD_WILSON_PREFETCH 0
+#endif
 
 namespace lqcd {
 
@@ -28,7 +39,7 @@ enum WilsonEpilogue {
     WE_PLAIN = 0,     // out = D in on one parity                               (lqcd_dslash)
     WE_M = 1,         // out = in - kappa D in, full lattice
     WE_M_NORM = 2,    // the same + tt = |out|^2, alpha = rr/tt                 (S1, S2: <p,Ap> = |Mp|^2)
-    WE_CGUPDATE = 3,  // Ap = in - kappa D^+ in; x += alpha p; r -= alpha Ap; |r|^2   (S3)
+    WE_CGUPDATE = 3,  // Ap = in - kappa D^+ in; r -= alpha Ap; |r|^2   (S3; its x += alpha p: cg_xpupdate_kernel)
     WE_RESIDUAL = 4,  // |b - (in - kappa D^+ in)|^2                            (S7)
     // One-parity kernels of the even-odd (Schur) preconditioned solver, SURVEY.md 8(f) row 4.  `p` is the
     // site-diagonal operand on the output parity, `kappa` carries the coefficient c of  d = p + c * (D in):
@@ -36,7 +47,7 @@ enum WilsonEpilogue {
     // reconstruction, c = -kappa for the rows of M itself.
     WE_EO_XPAY = 5,       // out = d
     WE_EO_XPAY_NORM = 6,  // out = d, tt = |d|^2, alpha = rr/tt                 (<p, Mhat^+ Mhat p> = |Mhat p|^2)
-    WE_EO_CGUPDATE = 7,   // Ap = d; x += alpha q; r -= alpha Ap; |r|^2         (q = the search direction, in `b`)
+    WE_EO_CGUPDATE = 7,   // Ap = d; r -= alpha Ap; |r|^2                       (x += alpha q: cg_xpupdate_kernel)
     WE_EO_RESIDUAL = 8    // |b - d|^2 and |b|^2 of one parity, set (flag = 0) or added (flag = 1)
 };
 __host__ __device__ constexpr bool wilson_one_parity(int epi) { return epi == WE_PLAIN || epi >= WE_EO_XPAY; }
@@ -164,33 +175,49 @@ __device__ __forceinline__ void wilson_epilogue(const WilsonArgs& a, bool active
         return;
     }
     if (EPI >= WE_EO_XPAY) {
-        // one-parity forms: d = p + c * acc
+        // one-parity forms: d = p + c * acc (operands loaded in batches before the stores, as below)
         double local[2] = { 0.0, 0.0 };
-        const double alpha = (EPI == WE_EO_CGUPDATE && active) ? a.sc->alpha : 0.0;
         if (active) {
+            if (EPI == WE_EO_CGUPDATE) {
+                // r -= alpha Ap, |r|^2; x += alpha q is done by cg_xpupdate_kernel (q = the search direction it updates)
+                const double alpha = a.sc->alpha;
+                constexpr int NB = LQCD_WILSON_EPI_BATCH_U;
 #pragma unroll
-            for (int k = 0; k < 12; ++k) {
-                const size_t i = (size_t)k * V + gsite;
-                const cplx c0 = a.p[i];
-                const cplx d = cmake(fma(a.kappa, acc[k / 3][k % 3].x, c0.x), fma(a.kappa, acc[k / 3][k % 3].y, c0.y));
-                if (EPI == WE_EO_XPAY || EPI == WE_EO_XPAY_NORM) {
-                    st_vec(a.out + i, d);
-                    if (EPI == WE_EO_XPAY_NORM) local[0] += cnorm2(d);
-                } else if (EPI == WE_EO_CGUPDATE) {
-                    const cplx qv = a.b[i];
-                    cplx xv = a.x[i], rv = a.r[i];
-                    xv.x = fma(alpha, qv.x, xv.x);
-                    xv.y = fma(alpha, qv.y, xv.y);
-                    rv.x = fma(-alpha, d.x, rv.x);
-                    rv.y = fma(-alpha, d.y, rv.y);
-                    a.x[i] = xv;
-                    a.r[i] = rv;
-                    local[0] += cnorm2(rv);
-                } else {  // WE_EO_RESIDUAL
-                    const cplx bv = a.b[i];
-                    const double re = bv.x - d.x, im = bv.y - d.y;
-                    local[0] += fma(re, re, im * im);
-                    local[1] += cnorm2(bv);
+                for (int h = 0; h < 12 / NB; ++h) {
+                    cplx c0[NB], rv[NB];
+#pragma unroll
+                    for (int j = 0; j < NB; ++j) {
+                        const size_t i = (size_t)(h * NB + j) * V + gsite;
+                        c0[j] = a.p[i];
+                        rv[j] = a.r[i];
+                    }
+#pragma unroll
+                    for (int j = 0; j < NB; ++j) {
+                        const int k = h * NB + j;
+                        const cplx d = cmake(fma(a.kappa, acc[k / 3][k % 3].x, c0[j].x), fma(a.kappa, acc[k / 3][k % 3].y, c0[j].y));
+                        rv[j].x = fma(-alpha, d.x, rv[j].x);
+                        rv[j].y = fma(-alpha, d.y, rv[j].y);
+                        a.r[(size_t)k * V + gsite] = rv[j];
+                        local[0] += cnorm2(rv[j]);
+                    }
+                }
+            } else {
+                cplx c0[12];
+#pragma unroll
+                for (int k = 0; k < 12; ++k) c0[k] = a.p[(size_t)k * V + gsite];
+#pragma unroll
+                for (int k = 0; k < 12; ++k) {
+                    const size_t i = (size_t)k * V + gsite;
+                    const cplx d = cmake(fma(a.kappa, acc[k / 3][k % 3].x, c0[k].x), fma(a.kappa, acc[k / 3][k % 3].y, c0[k].y));
+                    if (EPI == WE_EO_XPAY || EPI == WE_EO_XPAY_NORM) {
+                        st_vec(a.out + i, d);
+                        if (EPI == WE_EO_XPAY_NORM) local[0] += cnorm2(d);
+                    } else {  // WE_EO_RESIDUAL
+                        const cplx bv = a.b[i];
+                        const double re = bv.x - d.x, im = bv.y - d.y;
+                        local[0] += fma(re, re, im * im);
+                        local[1] += cnorm2(bv);
+                    }
                 }
             }
         }
@@ -202,7 +229,10 @@ __device__ __forceinline__ void wilson_epilogue(const WilsonArgs& a, bool active
             });
         } else if (EPI == WE_EO_CGUPDATE) {
             double* hist = a.hist;
-            grid_sum<BLOCK>(local[0], a.rs, [sc, hist](double rr_new) { cg_after_update(sc, hist, rr_new); });
+            grid_sum<BLOCK>(local[0], a.rs, [sc, hist](double rr_new) {
+                cg_after_update(sc, hist, rr_new);
+                sc->xdue = 1;
+            });
         } else if (EPI == WE_EO_RESIDUAL) {
             const int add = a.flag;
             grid_sum_n<BLOCK, 2>(local, a.rs, [sc, add](const double (&tot)[2]) {
@@ -212,30 +242,62 @@ __device__ __forceinline__ void wilson_epilogue(const WilsonArgs& a, bool active
         }
         return;
     }
-    // M-type: m = in(x) - kappa * acc
+    // M-type: m = in(x) - kappa * acc.  The operands of a batch are all loaded before the first store of that
+    // batch: `in`, `out`, `r` may alias as far as the compiler can tell, so a load placed after a store waits
+    // for it -- component by component that was twelve serial round trips to L2 per thread (ncu, round 2).
     double local = 0.0;
-    const double alpha = (EPI == WE_CGUPDATE && active) ? a.sc->alpha : 0.0;
-    if (active) {
+    if (EPI == WE_M || EPI == WE_M_NORM) {
+        if (active) {
+            constexpr int NB = LQCD_WILSON_EPI_BATCH_M;
 #pragma unroll
-        for (int k = 0; k < 12; ++k) {
-            const size_t i = (size_t)k * V + gsite;
-            const cplx c0 = a.in[i];
-            const cplx m = cmake(fma(-a.kappa, acc[k / 3][k % 3].x, c0.x), fma(-a.kappa, acc[k / 3][k % 3].y, c0.y));
-            if (EPI == WE_M || EPI == WE_M_NORM) {
-                st_vec(a.out + i, m);
-                if (EPI == WE_M_NORM) local += cnorm2(m);
-            } else if (EPI == WE_CGUPDATE) {
-                const cplx pv = a.p[i];
-                cplx xv = a.x[i], rv = a.r[i];
-                xv.x = fma(alpha, pv.x, xv.x);
-                xv.y = fma(alpha, pv.y, xv.y);
-                rv.x = fma(-alpha, m.x, rv.x);
-                rv.y = fma(-alpha, m.y, rv.y);
-                a.x[i] = xv;
-                a.r[i] = rv;
-                local += cnorm2(rv);
-            } else {  // WE_RESIDUAL
-                const cplx bv = a.b[i];
+            for (int h = 0; h < 12 / NB; ++h) {
+                cplx c0[NB];
+#pragma unroll
+                for (int j = 0; j < NB; ++j) c0[j] = a.in[(size_t)(h * NB + j) * V + gsite];
+#pragma unroll
+                for (int j = 0; j < NB; ++j) {
+                    const int k = h * NB + j;
+                    const cplx m = cmake(fma(-a.kappa, acc[k / 3][k % 3].x, c0[j].x), fma(-a.kappa, acc[k / 3][k % 3].y, c0[j].y));
+                    st_vec(a.out + (size_t)k * V + gsite, m);
+                    if (EPI == WE_M_NORM) local += cnorm2(m);
+                }
+            }
+        }
+    } else if (EPI == WE_CGUPDATE) {
+        // r -= alpha Ap, |r|^2.  x += alpha p is done by the vector kernel that follows (cg_xpupdate_kernel): it reads p
+        // anyway, so the search direction is not read here at all (192 B per site less than in round 1).
+        if (active) {
+            const double alpha = a.sc->alpha;
+            constexpr int NB = LQCD_WILSON_EPI_BATCH_U;
+#pragma unroll
+            for (int h = 0; h < 12 / NB; ++h) {
+                cplx c0[NB], rv[NB];
+#pragma unroll
+                for (int j = 0; j < NB; ++j) {
+                    const size_t i = (size_t)(h * NB + j) * V + gsite;
+                    c0[j] = a.in[i];
+                    rv[j] = a.r[i];
+                }
+#pragma unroll
+                for (int j = 0; j < NB; ++j) {
+                    const int k = h * NB + j;
+                    const cplx m = cmake(fma(-a.kappa, acc[k / 3][k % 3].x, c0[j].x), fma(-a.kappa, acc[k / 3][k % 3].y, c0[j].y));
+                    rv[j].x = fma(-alpha, m.x, rv[j].x);
+                    rv[j].y = fma(-alpha, m.y, rv[j].y);
+                    a.r[(size_t)k * V + gsite] = rv[j];
+                    local += cnorm2(rv[j]);
+                }
+            }
+        }
+    } else {  // WE_RESIDUAL
+        if (active) {
+            cplx c0[12];
+#pragma unroll
+            for (int k = 0; k < 12; ++k) c0[k] = a.in[(size_t)k * V + gsite];
+#pragma unroll
+            for (int k = 0; k < 12; ++k) {
+                const cplx m = cmake(fma(-a.kappa, acc[k / 3][k % 3].x, c0[k].x), fma(-a.kappa, acc[k / 3][k % 3].y, c0[k].y));
+                const cplx bv = a.b[(size_t)k * V + gsite];
                 const double re = bv.x - m.x, im = bv.y - m.y;
                 local += fma(re, re, im * im);
             }
@@ -249,7 +311,10 @@ __device__ __forceinline__ void wilson_epilogue(const WilsonArgs& a, bool active
         });
     } else if (EPI == WE_CGUPDATE) {
         double* hist = a.hist;
-        grid_sum<BLOCK>(local, a.rs, [sc, hist](double rr_new) { cg_after_update(sc, hist, rr_new); });
+        grid_sum<BLOCK>(local, a.rs, [sc, hist](double rr_new) {
+            cg_after_update(sc, hist, rr_new);
+            sc->xdue = 1;  // the x += alpha p of this iteration is still to be done
+        });
     } else if (EPI == WE_RESIDUAL) {
         grid_sum<BLOCK>(local, a.rs, [sc](double res2) { sc->res2 = res2; });
     }
@@ -273,6 +338,16 @@ __global__ void __launch_bounds__(BLOCK, LQCD_WILSON_MINB) wilson_dslash_kernel(
     for (int s = 0; s < 4; ++s)
 #pragma unroll
         for (int c = 0; c < 3; ++c) acc[s][c] = czero<cplx>();
+#if LQCD_WILSON_PREFETCH
+    // The residual at the own site is first needed after the eight hops: ask L2 for its lines now (one request
+    // per 128-byte line, no register held), so that the epilogue's loads find them there.
+    if (EPI == WE_CGUPDATE || EPI == WE_EO_CGUPDATE) {
+        if (active && (threadIdx.x & 7) == 0) {
+#pragma unroll
+            for (int k = 0; k < 12; ++k) prefetch_l2(a.r + (size_t)k * a.g.V + gsite);
+        }
+    }
+#endif
     if (active) {
         const Site st = decode_site(a.g, parity, e);
         wilson_dir<0, DAGGER, RECON, LINKS>(a, st, parity, acc);
