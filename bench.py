@@ -129,6 +129,49 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def workload_name(cfg):
+    return "%s: %s %s, %s links, %s=%g, tol=%g, fp64" % (
+        cfg["name"], "x".join(map(str, cfg["dims"])), cfg["fermion"], cfg["links"],
+        "mass" if cfg["fermion"] == "staggered" else "kappa", cfg["param"], cfg["tol"])
+
+
+def config_dict(args, cfg, world):
+    """The `config` object of the JSON line: the same keys and values in our arm and in the reference arm
+    (what the reference arm samples of the workload is said in its cpu_baseline.sample)."""
+    v = synth.volume(cfg["dims"])
+    return {"workload": workload_name(cfg), "precision": args.precision, "reconstruct": args.recon,
+            "cg_mode": args.cg_mode, "check_every": args.check_every,
+            "parallelism": "replicas x%d (independent right-hand sides)" % world,
+            "l2_policy": "inputs larger than L2 (%.0f MB of links per Dslash), no flush" % (v * 576 / 1e6)}
+
+
+def oracle_dslash_times(cfg, u, b, budget_s=4.0):
+    """The oracle's hopping term alone (SURVEY 8(d) timing protocol; the paper's fmv/fmtv):
+    microseconds per call on all host cores and on one thread, beside the GPU's dslash.us_per_call."""
+    import oracle
+    f = 0 if cfg["fermion"] == "staggered" else 1
+    nbytes = (STAG_DSLASH_BYTES if f == 0 else WILSON_DSLASH_BYTES) * (synth.volume(cfg["dims"]) // 2)
+    all_threads = oracle.num_threads()
+    out = {"cores": all_threads}
+    for label, nthr in (("all_cores", all_threads), ("one_thread", 1)):
+        oracle.set_threads(nthr)
+        try:
+            t0 = time.perf_counter()
+            oracle.dslash(cfg["dims"], f, u, 1, b)
+            t1 = time.perf_counter() - t0
+            reps = max(1, min(50, int(budget_s / 2 / max(t1, 1e-6))))
+            t0 = time.perf_counter()
+            for _ in range(reps):
+                oracle.dslash(cfg["dims"], f, u, 1, b)
+            sec = (time.perf_counter() - t0) / reps
+        finally:
+            oracle.set_threads(all_threads)
+        out["us_per_call_" + label] = sec * 1e6
+        out["GBps_" + label] = nbytes / sec / 1e9
+        out["reps_" + label] = reps
+    return out
+
+
 def oracle_arm(cfg, u, b, steps, warmup, target_seconds=6.0):
     """The oracle as it stands on the host cores: each step = `n_it` CG iterations (tol = 0)."""
     import oracle
@@ -172,6 +215,51 @@ def slab_group_variant(slab_mod, cfg, ug, bg, R, args, maxiter):
                 "GBps": cg_bytes(cfg, it_g, args.recon) / (ms_g * 1e-3) / 1e9}
     finally:
         grp.close()
+
+
+def slab_strong_variant(args, cfg, ranks, device, maxiter):
+    """One solve of cfg as N time-slabs, one per rank/GPU (collective: every rank calls it).  Returns a dict on every
+    rank; an {"error": ...} dict if anything fails on any rank."""
+    import torch
+    from paper_1311_2719_b200 import slab as sl
+    rank, world = ranks.rank, ranks.world
+    dims = cfg["dims"]
+    out, s = None, None
+    try:
+        if dims[3] % world or (dims[3] // world) % 2 or dims[3] // world < 2:
+            raise ValueError("L3 = %d cannot be cut into %d even slabs" % (dims[3], world))
+        ug = torch.from_numpy(synth.gauge_field(dims, cfg["links"], cfg["seed"]))
+        bg = torch.from_numpy(synth.source(dims, cfg["fermion"], cfg["seed"]))
+        s = sl.Slab(dims, rank, world, device=device)
+        s.set_option(sl.OPT_RECONSTRUCT, args.recon)
+        s.set_option(sl.OPT_CHECK_EVERY, args.check_every)
+        s.set_option(sl.OPT_TIMEOUT_MS, 10000)
+        s.connect_ipc()
+        s.load_gauge(sl.local_gauge(ug, dims, rank, world).to(device), sl.u3_below_from_global(ug, dims, rank, world).to(device))
+        b_dev, x_dev = sl.local_vector(bg, dims, rank, world).to(device), s.new_vector()
+        del ug, bg
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for rep in range(2):   # one warm-up, one timed
+            ranks.barrier()
+            e0.record(s.stream)
+            _, it, res, st = s.cg_solve(cfg["param"], cfg["tol"], maxiter, b_dev, x_dev)
+            e1.record(s.stream)
+            ranks.barrier()
+        ms = ranks.max(e0.elapsed_time(e1))
+        sh = dims[0] * dims[1] * dims[2] // 2
+        out = {"time_to_solution_ms": ms, "iters": it, "true_residual": res, "converged": st == 0,
+               "GBps": cg_bytes(cfg, it, args.recon) / (ms * 1e-3) / 1e9, "scaling": "strong",
+               "nvlink_bytes_per_dslash_and_rank": 2 * sh * 48, "sync_points": s.sync_points(),
+               "note": "one system, T = %d time-slices per GPU; first multi-GPU run of this path: check against the N = 1 solve" % (dims[3] // world)}
+    except Exception as exc:  # noqa: BLE001
+        out = {"error": repr(exc)[:300]}
+    finally:
+        try:
+            if s is not None:
+                s.close()
+        except Exception:  # noqa: BLE001
+            pass
+    return out
 
 
 def slab_arm(args, cfg, workload, metric, ranks, device):
@@ -271,73 +359,12 @@ def slab_arm(args, cfg, workload, metric, ranks, device):
     return 0
 
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=3)
-    ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=3)
-    ap.add_argument("--cg-mode", default="graph", choices=["sync", "async", "graph"])
-    ap.add_argument("--check-every", type=int, default=8)
-    ap.add_argument("--dslash-reps", type=int, default=200)
-    ap.add_argument("--recon", type=int, default=18, choices=[18, 12],
-                    help="stored reals per link: 18 = all nine entries (the roofline workload), 12 = two rows")
-    ap.add_argument("--precision", default="f64", choices=["f64", "mixed"],
-                    help="f64 = the fp64 conjugate gradient (the headline); mixed = fp32 iterations + fp64 reliable updates")
-    ap.add_argument("--delta", type=float, default=0.1, help="reliable-update threshold of --precision mixed")
-    ap.add_argument("--no-variants", action="store_true", help="skip the extra recon-12 / mixed-precision solves")
-    ap.add_argument("--parallelism", default="replicas", choices=["replicas", "slab"],
-                    help="N > 1: replicas = independent right-hand sides per GPU (weak scaling, the default); "
-                         "slab = ONE system cut into time-slabs, halo exchange and sums through peer memory "
-                         "(strong scaling; include/lqcd_slab.h; staggered configs)")
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-e2e", action="store_true")
-    args = ap.parse_args()
-
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-
-    cfg = synth.config(args.config)
-    workload = "%s: %s %s, %s links, %s=%g, tol=%g, fp64" % (
-        cfg["name"], "x".join(map(str, cfg["dims"])), cfg["fermion"], cfg["links"],
-        "mass" if cfg["fermion"] == "staggered" else "kappa", cfg["param"], cfg["tol"])
-    metric = "CG solve effective HBM throughput (algorithmic bytes of Dslash + fused updates / time-to-solution)"
-
-    # ------------------------------------------------------------------ reference arm = the oracle
-    if args.impl == "reference":
-        if rank != 0:
-            return 0
-        u = synth.gauge_field(cfg["dims"], cfg["links"], cfg["seed"])
-        b = synth.source(cfg["dims"], cfg["fermion"], cfg["seed"])
-        r = oracle_arm(cfg, u, b, max(1, args.steps), max(0, args.warmup), target_seconds=8.0)
-        line = {"impl": "reference", "metric": metric, "value": r["value"], "unit": "GB/s", "n_gpus": 0,
-                "steps": args.steps, "warmup": args.warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True,
-                "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-                "config": {"workload": workload, "sample": r["sample"]},
-                "cpu_baseline": {"value": r["value"], "unit": "GB/s", "cores": r["cores"], "kind": "oracle",
-                                 "sample": r["sample"]},
-                "e2e": {"value": r["value"], "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-                "gpu_launches": 0}
-        print(json.dumps(line))
-        return 0
-
-    # ------------------------------------------------------------------ our arm
-    import torch
-    from paper_1311_2719_b200 import lqcd
-    from paper_1311_2719_b200.ranks import Ranks
-
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: the CUDA path is the only path")
-    torch.cuda.set_device(local_rank)
-    device = torch.device("cuda", local_rank)
-    ranks = Ranks(backend="nccl", device=device)
+def ours_line(args, cfg, metric, ranks, device, lqcd, torch, full=True):
+    """Our arm on one config: returns the JSON line (a dict) on every rank.  full = False (--all-configs):
+    no solver variants, no oracle timing."""
+    rank, world, local_rank = ranks.rank, ranks.world, ranks.local_rank
     barrier, max_over_ranks, sum_over_ranks = ranks.barrier, ranks.max, ranks.sum
-
-    if args.parallelism == "slab":
-        return slab_arm(args, cfg, workload, metric, ranks, device)
-
+    workload = workload_name(cfg)
     f = lqcd.STAGGERED if cfg["fermion"] == "staggered" else lqcd.WILSON
     u = synth.gauge_field(cfg["dims"], cfg["links"], cfg["seed"])
     b = synth.source(cfg["dims"], cfg["fermion"], ranks.rhs_seed(cfg["seed"]))   # one right-hand side per rank
@@ -434,7 +461,7 @@ def main():
 
     # ---- the other solver variants on the same workload: time-to-solution only (one warm-up, one timed solve)
     variants = None
-    if f == lqcd.STAGGERED and not args.no_variants:
+    if f == lqcd.STAGGERED and not args.no_variants and full:
         variants = {}
         for recon_v, prec_v in ((18, "f64"), (12, "f64"), (18, "mixed"), (12, "mixed")):
             if (recon_v, prec_v) == (args.recon, args.precision):
@@ -477,33 +504,125 @@ def main():
 
     # ---- the oracle beside it (rank 0, N = 1 only)
     cpu = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and full:
         r = oracle_arm(cfg, u, b, steps=2, warmup=0, target_seconds=6.0)
-        cpu = {"value": r["value"], "unit": "GB/s", "cores": r["cores"], "kind": "oracle", "sample": r["sample"]}
+        cpu = {"value": r["value"], "unit": "GB/s", "cores": r["cores"], "kind": "oracle", "sample": r["sample"],
+               "dslash": oracle_dslash_times(cfg, u, b)}   # per call, all cores and one thread, beside dslash.us_per_call
 
-    if rank == 0:
-        line = {
-            "metric": metric, "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps,
-            "warmup": max(args.warmup, 3), "ms_per_step": ms_solve, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f64" if not mixed else "f32 iterations + f64 reliable updates",
-            "data": "synthetic",
-            "config": {"workload": workload, "precision": args.precision, "reconstruct": args.recon, "cg_mode": args.cg_mode, "check_every": args.check_every,
-                       "parallelism": "replicas x%d (independent right-hand sides)" % world,
-                       "l2_policy": "inputs larger than L2 (%.0f MB of links per Dslash), no flush" % (v * 576 / 1e6)},
-            "cg": {"time_to_solution_ms": ms_solve, "iters": iters, "reliable_updates": updates if mixed else None,
-                   "true_residual": res,
-                   "us_per_iteration": ms_solve * 1e3 / max(iters, 1)},
-            "dslash": {"us_per_call": us_dslash, "GBps": achieved, "GFLOPs": dflops * sites_out / (us_dslash * 1e-6) / 1e9,
-                       "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS, "reps": args.dslash_reps},
-            "roofline": {"bound": "hbm", "kernel": "stag_dslash_kernel<SE_PLAIN>" if f == lqcd.STAGGERED else
-                         "wilson_dslash_kernel<WE_PLAIN>", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": achieved / peak, "peak_source": peak_src, "traffic": None,
-                         "bytes_per_site": dbytes, "sites_per_launch": sites_out},
-            "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "cpu_baseline": cpu, "variants": variants,
-        }
-        line["roofline"]["traffic"] = ncu_traffic("%s_dslash_plain%s" % (cfg["name"], "" if args.recon == 18 else "_recon12"))
-        print(json.dumps(line))
+    line = {
+        "metric": metric, "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms_solve, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64" if not mixed else "f32 iterations + f64 reliable updates",
+        "data": "synthetic",
+        "config": config_dict(args, cfg, world),
+        "cg": {"time_to_solution_ms": ms_solve, "iters": iters, "reliable_updates": updates if mixed else None,
+               "true_residual": res,
+               "us_per_iteration": ms_solve * 1e3 / max(iters, 1)},
+        "dslash": {"us_per_call": us_dslash, "GBps": achieved, "GFLOPs": dflops * sites_out / (us_dslash * 1e-6) / 1e9,
+                   "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS, "reps": args.dslash_reps},
+        "roofline": {"bound": "hbm", "kernel": "stag_dslash_kernel<SE_PLAIN>" if f == lqcd.STAGGERED else
+                     "wilson_dslash_kernel<WE_PLAIN>", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                     "frac": achieved / peak, "peak_source": peak_src, "traffic": None, "traffic_source": None,
+                     "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
+                     "note": "peak = a copy (half its bytes are writes); this kernel is 96 % reads and its 48 B/site input is the "
+                             "previous launch's output (L2-resident in the ping-pong sweep), so frac can exceed 1: "
+                             "without that input 1200/1248 of it, on ncu DRAM bytes traffic/time",
+                     "bytes_per_site": dbytes, "sites_per_launch": sites_out},
+        "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "cpu_baseline": cpu, "variants": variants,
+    }
+    line["roofline"]["traffic"] = ncu_traffic("%s_dslash_plain%s" % (cfg["name"], "" if args.recon == 18 else "_recon12"))
+    if line["roofline"]["traffic"] is not None:
+        line["roofline"]["traffic_source"] = "profiles/traffic.csv (ncu --set full, builder-run; not measured by this run)"
+    if world > 1 and full and f == lqcd.STAGGERED and not mixed:
+        # N > 1: replicas stay the headline (BASELINE.json: everything runs on one GPU); beside it ONE solve of the same
+        # system cut into N time-slabs through lqcd_slab_cg_solve (IPC-mapped mailboxes, halo stores and sums through
+        # peer memory: what replaces the paper's host-staged MPI_ALLGATHER).  First run on real
+        # peers: bounded waits (LQCD_ECOMM) and try/except keep a failure out of the headline line.
+        sv = slab_strong_variant(args, cfg, ranks, device, maxiter)
+        if rank == 0:
+            line["variants"] = dict(line["variants"] or {}, **{"slab_strong_x%d" % world: sv})
     lat.close()
+    return line
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--cg-mode", default="graph", choices=["sync", "async", "graph"])
+    ap.add_argument("--check-every", type=int, default=8)
+    ap.add_argument("--dslash-reps", type=int, default=200)
+    ap.add_argument("--recon", type=int, default=18, choices=[18, 12],
+                    help="stored reals per link: 18 = all nine entries (the roofline workload), 12 = two rows")
+    ap.add_argument("--precision", default="f64", choices=["f64", "mixed"],
+                    help="f64 = the fp64 conjugate gradient (the headline); mixed = fp32 iterations + fp64 reliable updates")
+    ap.add_argument("--delta", type=float, default=0.1, help="reliable-update threshold of --precision mixed")
+    ap.add_argument("--no-variants", action="store_true", help="skip the extra recon-12 / mixed-precision solves")
+    ap.add_argument("--parallelism", default="replicas", choices=["replicas", "slab"],
+                    help="N > 1: replicas = independent right-hand sides per GPU (weak scaling, the default); "
+                         "slab = ONE system cut into time-slabs, halo exchange and sums through peer memory "
+                         "(strong scaling; include/lqcd_slab.h; staggered configs)")
+    ap.add_argument("--all-configs", action="store_true",
+                    help="the five BASELINE.json configs in one run (no variants, no oracle timing): one JSON line with a list")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    cfg = synth.config(args.config)
+    workload = workload_name(cfg)
+    metric = "CG solve effective HBM throughput (algorithmic bytes of Dslash + fused updates / time-to-solution)"
+
+    # ------------------------------------------------------------------ reference arm = the oracle
+    if args.impl == "reference":
+        if rank != 0:
+            return 0
+        u = synth.gauge_field(cfg["dims"], cfg["links"], cfg["seed"])
+        b = synth.source(cfg["dims"], cfg["fermion"], cfg["seed"])
+        r = oracle_arm(cfg, u, b, max(1, args.steps), max(0, args.warmup), target_seconds=8.0)
+        line = {"impl": "reference", "metric": metric, "value": r["value"], "unit": "GB/s", "n_gpus": 0,
+                "steps": args.steps, "warmup": args.warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": config_dict(args, cfg, 1),
+                "cpu_baseline": {"value": r["value"], "unit": "GB/s", "cores": r["cores"], "kind": "oracle",
+                                 "sample": r["sample"], "dslash": oracle_dslash_times(cfg, u, b)},
+                "e2e": {"value": r["value"], "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                "gpu_launches": 0}
+        print(json.dumps(line))
+        return 0
+
+    # ------------------------------------------------------------------ our arm
+    import torch
+    from paper_1311_2719_b200 import lqcd
+    from paper_1311_2719_b200.ranks import Ranks
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the CUDA path is the only path")
+    torch.cuda.set_device(local_rank)
+    device = torch.device("cuda", local_rank)
+    ranks = Ranks(backend="nccl", device=device)
+    barrier, max_over_ranks, sum_over_ranks = ranks.barrier, ranks.max, ranks.sum
+
+    if args.parallelism == "slab":
+        return slab_arm(args, cfg, workload, metric, ranks, device)
+
+    if args.all_configs:
+        # one process, the five BASELINE.json configs one after the other (no variants, no oracle timing):
+        # the table of profiles/ is written from this one line
+        lines = [ours_line(args, synth.config(n), metric, ranks, device, lqcd, torch, full=False) for n in (1, 2, 3, 4, 5)]
+        if rank == 0:
+            print(json.dumps({"metric": metric, "unit": "GB/s", "n_gpus": world, "all_configs": lines}))
+        ranks.close()
+        return 0
+    line = ours_line(args, cfg, metric, ranks, device, lqcd, torch, full=True)
+    if rank == 0:
+        print(json.dumps(line))
     ranks.close()
     return 0
 

@@ -25,6 +25,10 @@ constexpr int kStagBlock = 128;
 #define LQCD_WILSON_BLOCK 128
 #endif
 constexpr int kWilsonBlock = LQCD_WILSON_BLOCK;
+#ifndef LQCD_F32X2_BLOCK
+#define LQCD_F32X2_BLOCK 128
+#endif
+constexpr int kF32x2Block = LQCD_F32X2_BLOCK;  // threads per block of the two-sites-per-thread fp32 kernels
 constexpr int kVecBlock = 256;
 constexpr int kReorderTile = 64;
 constexpr size_t kAlign = 256;
@@ -222,11 +226,11 @@ template <int EPI>
 int launch_stag_f(lqcd_ctx* ctx, const StagArgsF& a)
 {
     if (ctx->f32_pairs && ctx->g.Lh % 2 == 0) {  // two sites per thread, 128-bit loads (stag_dslash_f32x2.cuh)
-        const unsigned int grid2 = blocks_for((size_t)ctx->g.Vh / 2, kStagBlock);
+        const unsigned int grid2 = blocks_for((size_t)ctx->g.Vh / 2, kF32x2Block);
         if (ctx->recon == 12)
-            stag_dslash_f32x2_kernel<EPI, kStagBlock, 12><<<grid2, kStagBlock, 0, ctx->stream>>>(a);
+            stag_dslash_f32x2_kernel<EPI, kF32x2Block, 12><<<grid2, kF32x2Block, 0, ctx->stream>>>(a);
         else
-            stag_dslash_f32x2_kernel<EPI, kStagBlock, 18><<<grid2, kStagBlock, 0, ctx->stream>>>(a);
+            stag_dslash_f32x2_kernel<EPI, kF32x2Block, 18><<<grid2, kF32x2Block, 0, ctx->stream>>>(a);
         LQCD_LAUNCH_CHECK();
         return LQCD_OK;
     }

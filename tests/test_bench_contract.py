@@ -40,6 +40,15 @@ def test_reference_arm_prints_the_contract_line():
     assert line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["cores"] >= 1
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["e2e"]["d2h_bytes_per_step"] == 0
     assert "workload" in line["config"] and "cfg1" in line["config"]["workload"]
+    # both arms carry the same config keys (what the reference arm samples is said in cpu_baseline.sample)
+    import argparse
+    import bench
+    from paper_1311_2719_b200 import synth
+    ours = bench.config_dict(argparse.Namespace(precision="f64", recon=18, cg_mode="graph", check_every=8), synth.config(1), 1)
+    assert line["config"] == ours
+    # the oracle's hopping term alone, per call, on all cores and on one thread (SURVEY 8(d) timing protocol)
+    d = line["cpu_baseline"]["dslash"]
+    assert d["us_per_call_all_cores"] > 0 and d["us_per_call_one_thread"] > 0 and d["cores"] == line["cpu_baseline"]["cores"]
 
 
 def test_reference_arm_other_ranks_exit_quietly():
