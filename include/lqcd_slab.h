@@ -20,8 +20,9 @@
  * PAPER.md:110-124): per Dslash a rank needs one time-slice of the input vector from each
  * neighbour (sh*48 bytes per face).  The kernel that PRODUCES a vector stores its two boundary
  * slices straight into the neighbours' ghost faces through peer memory (NVLink); inner products
- * travel as one partial per rank into every rank's slot array and are added in rank order, so every
- * rank holds bit-identical scalars.  A synchronisation point (signal, bounded wait, combine) runs in
+ * travel as one partial per rank into every rank's mailbox -- two 64-bit words, each tagged with the
+ * number of the synchronisation point, so that no fence has to order "data" before "flag" -- and are
+ * added in rank order, so every rank holds bit-identical scalars.  A synchronisation point (signal, bounded wait, combine) runs in
  * the last block of the producing kernel when a rank drives its own slab, or as two tiny kernels in
  * the *_group calls; nothing goes through the host.  All of that memory is the rank's MAILBOX.
  *
@@ -82,8 +83,8 @@ int lqcd_slab_create(lqcd_slab **out, int L0, int L1, int L2, int L3, int rank, 
 int lqcd_slab_destroy(lqcd_slab *s);
 
 /* Device memory the caller provides (both 256-byte aligned): the private workspace (links, r, p, t,
- * reduction scratch) and the mailbox (flags, slots, ghost faces) the peers store into.  The call zeroes
- * the mailbox flags; every rank must have done so before any rank's first compute call (a host
+ * reduction scratch) and the mailbox (tagged words, ghost faces) the peers store into.  The call zeroes
+ * the mailbox words; every rank must have done so before any rank's first compute call (a host
  * barrier in the caller).  cuda_stream as in lqcd_set_workspace. */
 size_t lqcd_slab_workspace_bytes(const lqcd_slab *s);
 size_t lqcd_slab_mailbox_bytes(const lqcd_slab *s);

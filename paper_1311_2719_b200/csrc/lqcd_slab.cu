@@ -33,7 +33,7 @@ struct lqcd_slab {
     // workspace (private) byte offsets
     size_t off_gauge, off_gghost, off_r, off_p, off_t, off_sc, off_ss, off_ticket, off_partials, off_hist, ws_needed;
     // mailbox (peer-visible) byte offsets
-    size_t mb_flag, mb_slot, mb_ghost, mb_needed;
+    size_t mb_word, mb_ghost, mb_needed;
     size_t max_blocks;
     char* ws;
     char* mb;
@@ -109,6 +109,21 @@ unsigned int vec_grid(const lqcd_slab* s)
     if (b > cap) b = cap;
     if (b < 1) b = 1;
     return (unsigned int)b;
+}
+
+// Face-first walk of the slab vector kernels (slab_kernels.cuh): the face elements, one per thread, to the first
+// blocks of the grid -- at most half of it.
+SlabVecPlan vec_plan(const lqcd_slab* s, unsigned int grid)
+{
+    SlabVecPlan pl;
+    pl.n = s->nvec;
+    pl.nface = 6 * (size_t)s->sh < s->nvec ? 6 * (size_t)s->sh : s->nvec;
+    size_t fb = (pl.nface + kVecBlock - 1) / kVecBlock;
+    if (pl.nface == pl.n) fb = grid;               // no interior (T = 2): every block owns face elements
+    else if (fb > grid / 2) fb = grid / 2;
+    if (fb < 1) fb = 1;
+    pl.face_blocks = (int)fb;
+    return pl;
 }
 
 // The n slabs of a *_group call.
@@ -259,13 +274,9 @@ SlabSyncArgs sync_args(const lqcd_slab* s, int op, int nvals, double m2, double 
     a.rank = s->rank;
     a.nranks = s->nranks;
     a.nvals = nvals;
-    a.own.flag = (unsigned long long*)(s->mb + s->mb_flag);
-    a.own.slot = (double*)(s->mb + s->mb_slot);
+    a.own.word = (unsigned long long*)(s->mb + s->mb_word);
     a.own.ghost = (cplx*)(s->mb + s->mb_ghost);
-    for (int r = 0; r < s->nranks; ++r) {
-        a.peer_flag[r] = (unsigned long long*)(s->peer[r] + s->mb_flag);
-        a.peer_slot[r] = (double*)(s->peer[r] + s->mb_slot);
-    }
+    for (int r = 0; r < s->nranks; ++r) a.peer_word[r] = (unsigned long long*)(s->peer[r] + s->mb_word);
     a.ss = s->ss();
     a.sc = s->sc();
     a.hist = s->hist();
@@ -454,7 +465,7 @@ int group_iteration(const Group& G, double mass, cplx* const* x)
         rc = use_device(s);
         if (rc) return rc;
         slab_cg_pupdate_kernel<kVecBlock><<<vec_grid(s), kVecBlock, 0, s->stream>>>(
-            s->r(), s->p(), s->nvec, push_next(s), s->sc(), s->ss(), s->rs(), sync_args(s, SLAB_OP_PP, 1, 0.0, 0.0, 0), fz ? 1 : 0);
+            s->r(), s->p(), vec_plan(s, vec_grid(s)), push_next(s), s->sc(), s->ss(), s->rs(), sync_args(s, SLAB_OP_PP, 1, 0.0, 0.0, 0), fz ? 1 : 0);
         SLAB_LAUNCH_CHECK();
     }
     return group_sync(G, SLAB_OP_PP, 1, 0.0, 0.0, 0, fz);
@@ -470,7 +481,7 @@ int group_cg(const Group& G, double mass, double tol, int maxiter, const cplx* c
         rc = use_device(s);
         if (rc) return rc;
         slab_cg_init_kernel<kVecBlock><<<vec_grid(s), kVecBlock, 0, s->stream>>>(
-            b[r], x[r], s->r(), s->p(), s->nvec, push_next(s), s->ss(), s->rs(), sync_args(s, SLAB_OP_INIT, 1, 0.0, tol, maxiter),
+            b[r], x[r], s->r(), s->p(), vec_plan(s, vec_grid(s)), push_next(s), s->ss(), s->rs(), sync_args(s, SLAB_OP_INIT, 1, 0.0, tol, maxiter),
             fused(G) ? 1 : 0);
         SLAB_LAUNCH_CHECK();
     }
@@ -637,8 +648,7 @@ int lqcd_slab_create(lqcd_slab** out, int L0, int L1, int L2, int L3, int rank, 
     c->ws_needed = off;
 
     off = 0;
-    c->mb_flag = off;   off += align_up(LQCD_SLAB_MAX_RANKS * sizeof(unsigned long long));
-    c->mb_slot = off;   off += align_up(2 * LQCD_SLAB_MAX_RANKS * 2 * sizeof(double));
+    c->mb_word = off;   off += align_up(2 * LQCD_SLAB_MAX_RANKS * 4 * sizeof(unsigned long long));
     c->mb_ghost = off;  off += align_up(2 * 2 * 3 * (size_t)c->sh * sizeof(cplx));
     c->mb_needed = off;
     *out = c;
@@ -690,7 +700,7 @@ int lqcd_slab_set_memory(lqcd_slab* s, void* workspace_dev, size_t workspace_byt
     s->gauge_loaded = false;
     s->seq = 0;
     SLAB_CUDA(cudaMemsetAsync(s->ws + s->off_sc, 0, align_up(sizeof(CgScalars)) + align_up(sizeof(SlabScalars)) + kAlign, s->stream));
-    SLAB_CUDA(cudaMemsetAsync(s->mb, 0, s->mb_ghost, s->stream));  // flags and slots
+    SLAB_CUDA(cudaMemsetAsync(s->mb, 0, s->mb_ghost, s->stream));  // the tagged words (tag 0 = no synchronisation point)
     SLAB_CUDA(cudaStreamSynchronize(s->stream));
     return LQCD_OK;
 }

@@ -7,10 +7,10 @@
 //   producer kernel   writes its vector, stores the two boundary time-slices of that vector into the
 //                     neighbour ranks' ghost faces (buffer seq & 1) through peer memory, and leaves
 //                     this rank's partial sum(s) in `part`;
-//   slab_signal       thread r: copies `part` into rank r's slot [seq & 1][me], fences at system scope,
-//                     then stores flag[me] = seq in rank r's mailbox;
-//   slab_wait_combine thread r: waits (bounded) until flag[r] >= seq in the own mailbox; then one
-//                     thread adds the slots in RANK ORDER -- every rank adds the same numbers in the
+//   slab_signal       thread r: stores `part`, as 64-bit words tagged with seq, into rank r's mailbox
+//                     [seq & 1][me] (slab_sync.cuh: the tag makes a separate flag and its fences unnecessary);
+//   slab_wait_combine thread r: waits (bounded) for rank r's words of this seq in the own mailbox; then one
+//                     thread adds the values in RANK ORDER -- every rank adds the same numbers in the
 //                     same order, so all ranks hold bit-identical scalars and take the same exit
 //                     decision -- and runs the scalar step of the CG.
 //   A rank that drives only its own slab runs signal + wait + combine in the LAST BLOCK of the producer
@@ -30,32 +30,11 @@ static __global__ void slab_signal_kernel(const SlabSyncArgs a)
     if ((int)threadIdx.x < a.nranks) slab_signal(a, a.ss->seq + 1, threadIdx.x);
 }
 
-static __global__ void slab_wait_combine_kernel(const SlabSyncArgs a)
-{
-    __shared__ int timed_out;
-    const unsigned long long seq = a.ss->seq + 1;
-    if (threadIdx.x == 0) timed_out = 0;
-    __syncthreads();
-    if ((int)threadIdx.x < a.nranks && !slab_wait(a, seq, threadIdx.x)) timed_out = 1;
-    __syncthreads();
-    if (threadIdx.x == 0) slab_combine(a, seq, timed_out != 0);
-}
+static __global__ void slab_wait_combine_kernel(const SlabSyncArgs a) { slab_sync_point(a, false); }
 
 // Both in one launch: what a rank that drives only its own slab enqueues (one process per GPU).
 // Never used by a group of several slabs on one stream, where every signal must precede every wait.
-static __global__ void slab_signal_wait_combine_kernel(const SlabSyncArgs a)
-{
-    __shared__ int timed_out;
-    const unsigned long long seq = a.ss->seq + 1;
-    if (threadIdx.x == 0) timed_out = 0;
-    __syncthreads();
-    if ((int)threadIdx.x < a.nranks) {
-        slab_signal(a, seq, threadIdx.x);
-        if (!slab_wait(a, seq, threadIdx.x)) timed_out = 1;
-    }
-    __syncthreads();
-    if (threadIdx.x == 0) slab_combine(a, seq, timed_out != 0);
-}
+static __global__ void slab_signal_wait_combine_kernel(const SlabSyncArgs a) { slab_sync_point(a, true); }
 
 
 // Where the two boundary time-slices of a slab vector go: element (c, e) of local slice 0 into the
@@ -67,25 +46,60 @@ struct SlabPush {
     int Vh;       // local sites of one parity
 };
 
-__device__ __forceinline__ bool slab_push_elem(const SlabPush& ph, size_t i, cplx v)
+// The vector kernels walk the n = 3 Vh elements in a FACE-FIRST order: virtual index v < 6 sh is an element of one
+// of the two boundary time-slices (face f = v / sh: colour f / 2, first or last slice), the rest is the interior.
+// The first `face_blocks` blocks of the grid own the face elements, one per thread where the grid allows: they store
+// into a neighbour's memory, must fence at system scope before they take the reduction ticket, and -- having a
+// fraction of the work of an interior block -- do so while the interior blocks are still streaming (round 1: the
+// fence sat on the kernel's tail, 28.6 us against 14.4 us for the same p-update without faces).
+struct SlabVecPlan {
+    size_t n, nface;   // elements, face elements (6 sh, or n if the slab has no interior)
+    int face_blocks;   // blocks [0, face_blocks) own the face elements, the others the interior
+};
+
+__device__ __forceinline__ void slab_vec_range(const SlabVecPlan& pl, size_t& v0, size_t& v1)
 {
-    const size_t c = i / (size_t)ph.Vh;
-    const size_t e = i - c * (size_t)ph.Vh;
-    const bool lo = e < (size_t)ph.sh, hi = e >= (size_t)(ph.Vh - ph.sh);
-    if (lo) ph.lo[c * ph.sh + e] = v;
-    if (hi) ph.hi[c * ph.sh + (e - (size_t)(ph.Vh - ph.sh))] = v;
-    return lo || hi;
+    if (gridDim.x == 1) {  // a single block walks everything, faces first
+        v0 = 0;
+        v1 = pl.n;
+        return;
+    }
+    if ((int)blockIdx.x < pl.face_blocks) {
+        const size_t per = (pl.nface + pl.face_blocks - 1) / pl.face_blocks;
+        v0 = (size_t)blockIdx.x * per;
+        v1 = v0 + per < pl.nface ? v0 + per : pl.nface;
+        if (v0 > pl.nface) v0 = pl.nface;
+    } else {
+        const size_t nint = pl.n - pl.nface, nb = gridDim.x - pl.face_blocks;
+        const size_t per = (nint + nb - 1) / nb;
+        v0 = pl.nface + (size_t)(blockIdx.x - pl.face_blocks) * per;
+        v1 = v0 + per < pl.n ? v0 + per : pl.n;
+        if (v0 > pl.n) v0 = pl.n;
+    }
 }
 
-// The vector kernels give every block one contiguous run of elements (not a grid-stride walk), so only
-// the few blocks whose run meets a boundary time-slice store into a neighbour's memory -- and only
-// those pay for a system-scope fence.
-__device__ __forceinline__ void slab_block_range(size_t n, size_t& i0, size_t& i1)
+// virtual index -> element index i = c Vh + e, and where (if anywhere) the element goes in the neighbours' ghosts
+__device__ __forceinline__ size_t slab_vec_elem(const SlabPush& ph, const SlabVecPlan& pl, size_t v, cplx*& peer_dst)
 {
-    const size_t per = (n + gridDim.x - 1) / gridDim.x;
-    i0 = (size_t)blockIdx.x * per;
-    i1 = i0 + per < n ? i0 + per : n;
-    if (i0 > n) i0 = n;
+    const size_t sh = (size_t)ph.sh, Vh = (size_t)ph.Vh;
+    peer_dst = nullptr;
+    if (v < pl.nface) {
+        if (Vh == 2 * sh) {  // T = 2: every site lies on a face, plain order; slice 0 -> lo, slice 1 -> hi
+            const size_t c = v / Vh, e = v - c * Vh;
+            peer_dst = e < sh ? ph.lo + c * sh + e : ph.hi + c * sh + (e - sh);
+            return v;
+        }
+        const size_t f = v / sh, k = v - f * sh, c = f >> 1;
+        if (f & 1) {
+            peer_dst = ph.hi + c * sh + k;
+            return c * Vh + (Vh - sh) + k;
+        }
+        peer_dst = ph.lo + c * sh + k;
+        return c * Vh + k;
+    }
+    const size_t w = v - pl.nface, per = Vh - 2 * sh;
+    const size_t c = w / per;
+    return c * Vh + sh + (w - c * per);
 }
 
 // Faces of a vector that no kernel of ours produced (a caller's input, or x before the final check).
@@ -108,21 +122,26 @@ __global__ void __launch_bounds__(BLOCK) slab_push_faces_kernel(const cplx* __re
 // S6 on a slab: p = r = b, x = 0, partial <b,b>; the faces of p go to the neighbours.
 template <int BLOCK>
 __global__ void __launch_bounds__(BLOCK) slab_cg_init_kernel(const cplx* __restrict__ b, cplx* __restrict__ x,
-                                                             cplx* __restrict__ r, cplx* __restrict__ p, size_t n,
+                                                             cplx* __restrict__ r, cplx* __restrict__ p, SlabVecPlan pl,
                                                              SlabPush ph, SlabScalars* ss, ReduceScratch rs,
                                                              const SlabSyncArgs sy, int fused)
 {
     double local = 0.0;
     bool wrote_peer = false;
-    size_t i0, i1;
-    slab_block_range(n, i0, i1);
-    for (size_t i = i0 + threadIdx.x; i < i1; i += BLOCK) {
-        const cplx v = b[i];
-        r[i] = v;
-        p[i] = v;
+    size_t v0, v1;
+    slab_vec_range(pl, v0, v1);
+    for (size_t v = v0 + threadIdx.x; v < v1; v += BLOCK) {
+        cplx* dst;
+        const size_t i = slab_vec_elem(ph, pl, v, dst);
+        const cplx val = b[i];
+        r[i] = val;
+        p[i] = val;
         x[i] = cmake(0.0, 0.0);
-        wrote_peer |= slab_push_elem(ph, i, v);
-        local += cnorm2(v);
+        if (dst) {
+            *dst = val;
+            wrote_peer = true;
+        }
+        local += cnorm2(val);
     }
     if (fused)
         grid_sum_block<BLOCK>(local, wrote_peer, rs, [&sy](double bb) { slab_sync_tail<BLOCK>(sy, bb); });
@@ -132,7 +151,7 @@ __global__ void __launch_bounds__(BLOCK) slab_cg_init_kernel(const cplx* __restr
 
 // S5 on a slab: p = r + beta p, partial <p,p>; the faces of the new p go to the neighbours.
 template <int BLOCK>
-__global__ void __launch_bounds__(BLOCK) slab_cg_pupdate_kernel(const cplx* __restrict__ r, cplx* __restrict__ p, size_t n,
+__global__ void __launch_bounds__(BLOCK) slab_cg_pupdate_kernel(const cplx* __restrict__ r, cplx* __restrict__ p, SlabVecPlan pl,
                                                                 SlabPush ph, const CgScalars* sc, SlabScalars* ss,
                                                                 ReduceScratch rs, const SlabSyncArgs sy, int fused)
 {
@@ -140,15 +159,20 @@ __global__ void __launch_bounds__(BLOCK) slab_cg_pupdate_kernel(const cplx* __re
     const double beta = sc->beta;
     double local = 0.0;
     bool wrote_peer = false;
-    size_t i0, i1;
-    slab_block_range(n, i0, i1);
-    for (size_t i = i0 + threadIdx.x; i < i1; i += BLOCK) {
+    size_t v0, v1;
+    slab_vec_range(pl, v0, v1);
+    for (size_t v = v0 + threadIdx.x; v < v1; v += BLOCK) {
+        cplx* dst;
+        const size_t i = slab_vec_elem(ph, pl, v, dst);
         const cplx rv = r[i];
         cplx pv = p[i];
         pv.x = fma(beta, pv.x, rv.x);
         pv.y = fma(beta, pv.y, rv.y);
         p[i] = pv;
-        wrote_peer |= slab_push_elem(ph, i, pv);
+        if (dst) {
+            *dst = pv;
+            wrote_peer = true;
+        }
         local += cnorm2(pv);
     }
     if (fused)

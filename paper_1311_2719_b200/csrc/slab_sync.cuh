@@ -9,10 +9,18 @@ namespace lqcd {
 constexpr int kSlabMaxRanks = 16;
 
 // Mailbox of one rank (device memory the peers can address).  Byte offsets are computed on the host
-// by slab_mailbox_layout(); every rank uses the same layout for the same lattice and rank count.
+// by lqcd_slab_create; every rank uses the same layout for the same lattice and rank count.
+//
+// Sums and the "I have arrived" signal travel as TAGGED WORDS: a double goes out as two 64-bit stores, each
+// (sequence number << 32) | 32 bits of the value.  A 64-bit store is single-copy atomic, so a receiver that
+// sees the tag of the synchronisation point it waits for has the data that belongs to it -- no fence between
+// "slot" and "flag" on the sending side and none between "flag" and "slot" on the receiving side (round 1 paid
+// two system-scope fences per synchronisation point for that order).  Every synchronisation point sends at
+// least the two words of value 0, so the words are also the arrival signal for the ghost faces: those were made
+// visible system-wide by the blocks that stored them BEFORE they took the reduction ticket (grid_sum_block), and
+// the words are only sent after the last ticket.
 struct SlabMailbox {
-    unsigned long long* flag;  // [R]        flag[src] = last synchronisation point src has signalled
-    double* slot;              // [2][R][2]  partial sums of src at that point
+    unsigned long long* word;  // [2][R][4]  (seq & 1, source rank, {v0 lo, v0 hi, v1 lo, v1 hi})
     cplx* ghost;               // [2][2][3][sh]  (seq & 1, lo/hi, colour, site): the neighbours' boundary slices
 };
 
@@ -38,8 +46,7 @@ struct SlabSyncArgs {
     int rank, nranks;
     int nvals;                                     // partial sums carried by this point (0, 1 or 2)
     SlabMailbox own;
-    unsigned long long* peer_flag[kSlabMaxRanks];  // rank r's flag array
-    double* peer_slot[kSlabMaxRanks];              // rank r's slot array
+    unsigned long long* peer_word[kSlabMaxRanks];  // rank r's word array
     SlabScalars* ss;
     CgScalars* sc;
     double* hist;
@@ -49,14 +56,29 @@ struct SlabSyncArgs {
     unsigned long long timeout_ns;
 };
 
-// thread r < nranks: this rank's partial(s) into rank r's slot, then (after a system-scope fence) the flag.
-// The faces were stored by the producer kernel that precedes this one in the stream.
+__device__ __forceinline__ void st_sys_u64(unsigned long long* p, unsigned long long v)
+{
+    asm volatile("st.relaxed.sys.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ unsigned long long ld_acquire_sys_u64(const unsigned long long* p)
+{
+    unsigned long long v;
+    asm volatile("ld.acquire.sys.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+
+// thread r < nranks: this rank's partial(s), tagged with the number of the synchronisation point, into rank r's
+// mailbox.  The faces were stored -- and fenced at system scope -- by the producer's blocks before this runs.
 __device__ __forceinline__ void slab_signal(const SlabSyncArgs& a, unsigned long long seq, int r)
 {
-    double* dst = a.peer_slot[r] + ((seq & 1ull) * a.nranks + a.rank) * 2;
-    for (int k = 0; k < a.nvals; ++k) dst[k] = a.ss->part[k];
-    __threadfence_system();  // release: slots (and the producer's face stores) before the flag
-    *(volatile unsigned long long*)(a.peer_flag[r] + a.rank) = seq;
+    unsigned long long* dst = a.peer_word[r] + ((seq & 1ull) * a.nranks + a.rank) * 4;
+    const unsigned long long tag = seq << 32;
+    const int nv = a.nvals > 0 ? a.nvals : 1;  // a point without a sum still announces itself
+    for (int k = 0; k < nv; ++k) {
+        const unsigned long long bits = a.nvals > 0 ? (unsigned long long)__double_as_longlong(a.ss->part[k]) : 0ull;
+        st_sys_u64(dst + 2 * k, tag | (bits & 0xffffffffull));
+        st_sys_u64(dst + 2 * k + 1, tag | (bits >> 32));
+    }
 }
 
 __device__ __forceinline__ unsigned long long slab_now_ns()
@@ -66,21 +88,32 @@ __device__ __forceinline__ unsigned long long slab_now_ns()
     return t;
 }
 
-// thread r < nranks waits (bounded) for rank r's flag; returns false on a timeout.
-__device__ __forceinline__ bool slab_wait(const SlabSyncArgs& a, unsigned long long seq, int r)
+// thread r < nranks waits (bounded) for rank r's words of this synchronisation point and returns rank r's
+// values in val[]; false on a timeout.
+__device__ __forceinline__ bool slab_wait(const SlabSyncArgs& a, unsigned long long seq, int r, double val[2])
 {
-    const volatile unsigned long long* f = a.own.flag + r;
-    if (*f >= seq) return true;
-    const unsigned long long t0 = slab_now_ns();
-    while (*f < seq) {
-        if (slab_now_ns() - t0 > a.timeout_ns) return false;
-        __nanosleep(200);
+    const unsigned long long* src = a.own.word + ((seq & 1ull) * a.nranks + r) * 4;
+    const unsigned long long tag = (seq << 32) >> 32;
+    const int nv = a.nvals > 0 ? a.nvals : 1;
+    unsigned long long t0 = 0;
+    val[0] = val[1] = 0.0;
+    for (int k = 0; k < nv; ++k) {
+        unsigned long long lo, hi;
+        for (;;) {
+            lo = ld_acquire_sys_u64(src + 2 * k);
+            hi = ld_acquire_sys_u64(src + 2 * k + 1);
+            if ((lo >> 32) == tag && (hi >> 32) == tag) break;
+            if (t0 == 0) t0 = slab_now_ns();
+            if (slab_now_ns() - t0 > a.timeout_ns) return false;
+            __nanosleep(100);
+        }
+        val[k] = __longlong_as_double((long long)((hi << 32) | (lo & 0xffffffffull)));
     }
     return true;
 }
 
-// one thread: add the slots in rank order, run the scalar step, count the synchronisation point.
-__device__ __forceinline__ void slab_combine(const SlabSyncArgs& a, unsigned long long seq, bool timed_out)
+// one thread: add the ranks' values in rank order, run the scalar step, count the synchronisation point.
+__device__ __forceinline__ void slab_combine(const SlabSyncArgs& a, unsigned long long seq, bool timed_out, const double (*vals)[2])
 {
     a.ss->seq = seq;
     if (timed_out) {  // a peer never arrived: stop the solver instead of hanging the device
@@ -88,11 +121,9 @@ __device__ __forceinline__ void slab_combine(const SlabSyncArgs& a, unsigned lon
         a.sc->done = 1;
         return;
     }
-    __threadfence_system();  // acquire: the flags before the slots and the ghost faces
     double total[2] = { 0.0, 0.0 };
-    const volatile double* s = a.own.slot + (seq & 1ull) * a.nranks * 2;
     for (int q = 0; q < a.nranks; ++q)
-        for (int k = 0; k < a.nvals; ++k) total[k] += s[q * 2 + k];
+        for (int k = 0; k < a.nvals; ++k) total[k] += vals[q][k];
     CgScalars* sc = a.sc;
     switch (a.op) {
     case SLAB_OP_INIT: {
@@ -135,6 +166,26 @@ __device__ __forceinline__ void slab_combine(const SlabSyncArgs& a, unsigned lon
     }
 }
 
+// signal + bounded wait + combine by the threads of one block (at least nranks of them): the body of every form
+// of a synchronisation point.  do_signal = false: the signal was sent by an earlier launch (group calls).
+__device__ __forceinline__ void slab_sync_point(const SlabSyncArgs& a, bool do_signal)
+{
+    __shared__ int sp_timed_out;
+    __shared__ double sp_vals[kSlabMaxRanks][2];
+    const unsigned long long seq = a.ss->seq + 1;
+    if (threadIdx.x == 0) sp_timed_out = 0;
+    __syncthreads();
+    if ((int)threadIdx.x < a.nranks) {
+        if (do_signal) slab_signal(a, seq, threadIdx.x);
+        double v[2];
+        if (!slab_wait(a, seq, threadIdx.x, v)) sp_timed_out = 1;
+        sp_vals[threadIdx.x][0] = v[0];
+        sp_vals[threadIdx.x][1] = v[1];
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) slab_combine(a, seq, sp_timed_out != 0, sp_vals);
+}
+
 // The whole synchronisation point run by the LAST block of a producer kernel (`total` = this rank's
 // partial sum, known to every thread of that block): what a rank that drives only its own slab uses
 // instead of separate launches -- the halo exchange, the all-reduce and the scalar step of the CG
@@ -143,19 +194,9 @@ __device__ __forceinline__ void slab_combine(const SlabSyncArgs& a, unsigned lon
 template <int BLOCK>
 __device__ __forceinline__ void slab_sync_tail(const SlabSyncArgs& a, double total)
 {
-    __shared__ int tail_timed_out;
-    const unsigned long long seq = a.ss->seq + 1;
-    if (threadIdx.x == 0) {
-        tail_timed_out = 0;
-        a.ss->part[0] = total;
-    }
+    if (threadIdx.x == 0) a.ss->part[0] = total;
     __syncthreads();
-    if ((int)threadIdx.x < a.nranks) {
-        slab_signal(a, seq, threadIdx.x);
-        if (!slab_wait(a, seq, threadIdx.x)) tail_timed_out = 1;
-    }
-    __syncthreads();
-    if (threadIdx.x == 0) slab_combine(a, seq, tail_timed_out != 0);
+    slab_sync_point(a, true);
 }
 
 }  // namespace lqcd

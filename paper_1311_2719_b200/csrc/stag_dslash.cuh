@@ -185,8 +185,15 @@ __device__ __forceinline__ void stag_dslash_body(const StagArgs<C>& a, const Sla
         // converged earlier, or waiting for a reliable update: this (pre-enqueued) iteration is a no-op
         if (a.sc->done | a.sc->pause) return;
     }
-    const int e = blockIdx.x * BLOCK + threadIdx.x;
+    int e = blockIdx.x * BLOCK + threadIdx.x;
     const bool active = e < a.g.Vh;
+    if (SLAB) {
+        // Slab kernels walk the sites starting at the LAST time-slice (then slice 0, 1, ...): the blocks that store
+        // faces into a neighbour's memory -- and pay a system-scope fence for it before they take the reduction
+        // ticket -- are then the first to run instead of the last, and their fences are off the kernel's tail.
+        e += a.g.Vh - a.sl.sh;
+        if (e >= a.g.Vh) e -= a.g.Vh;
+    }
     const size_t Vh = (size_t)a.g.Vh;
     C acc[3] = { czero<C>(), czero<C>(), czero<C>() };
     int x3 = 0;
