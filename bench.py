@@ -194,8 +194,9 @@ def oracle_arm(cfg, u, b, steps, warmup, target_seconds=6.0):
                       % (n_it, cfg["name"], steps, sec), "ms_per_step": sec * 1e3, "iters_per_step": n_it}
 
 
-def slab_group_variant(slab_mod, cfg, ug, bg, R, args, maxiter):
-    """Time-to-solution of the R-slab decomposition with all slabs on this GPU (one warm-up + one timed solve)."""
+def slab_group_variant(slab_mod, cfg, ug, bg, R, args, maxiter, mixed=False):
+    """Time-to-solution of the R-slab decomposition with all slabs on this GPU (one warm-up + one timed solve);
+    mixed = True: the mixed-precision slab solver (lqcd_slab_cg_solve_mixed_group)."""
     import torch
     grp = slab_mod.SlabGroup(cfg["dims"], R, recon=args.recon)
     try:
@@ -207,12 +208,17 @@ def slab_group_variant(slab_mod, cfg, ug, bg, R, args, maxiter):
         for rep in range(2):
             torch.cuda.synchronize()
             g0.record(st)
-            _, it_g, res_g, st_g = grp.cg_solve(cfg["param"], cfg["tol"], maxiter, bs, xs)
+            if mixed:
+                _, it_g, nu_g, res_g, st_g = grp.cg_solve_mixed(cfg["param"], cfg["tol"], maxiter, bs, xs, delta=args.delta)
+            else:
+                _, it_g, res_g, st_g = grp.cg_solve(cfg["param"], cfg["tol"], maxiter, bs, xs)
+                nu_g = -1
             g1.record(st)
             torch.cuda.synchronize()
         ms_g = g0.elapsed_time(g1)
-        return {"time_to_solution_ms": ms_g, "iters": it_g, "true_residual": res_g, "converged": st_g == 0,
-                "GBps": cg_bytes(cfg, it_g, args.recon) / (ms_g * 1e-3) / 1e9}
+        return {"time_to_solution_ms": ms_g, "iters": it_g, "reliable_updates": nu_g if mixed else None,
+                "true_residual": res_g, "converged": st_g == 0,
+                "GBps": cg_bytes(cfg, it_g, args.recon, nu_g) / (ms_g * 1e-3) / 1e9}
     finally:
         grp.close()
 
@@ -501,6 +507,10 @@ def ours_line(args, cfg, metric, ranks, device, lqcd, torch, full=True):
                     variants["slab_group%d_on_one_gpu" % R] = slab_group_variant(slab_mod, cfg, ug, bg, R, args, maxiter)
                 except Exception as exc:  # noqa: BLE001
                     variants["slab_group%d_on_one_gpu" % R] = {"error": repr(exc)[:200]}
+            try:   # the mixed-precision slab solver (separate launches per synchronisation point), two slabs
+                variants["slab_group2_mixed_on_one_gpu"] = slab_group_variant(slab_mod, cfg, ug, bg, 2, args, maxiter, mixed=True)
+            except Exception as exc:  # noqa: BLE001
+                variants["slab_group2_mixed_on_one_gpu"] = {"error": repr(exc)[:200]}
 
     # ---- the oracle beside it (rank 0, N = 1 only)
     cpu = None

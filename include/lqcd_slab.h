@@ -110,6 +110,14 @@ int lqcd_slab_apply_MdagM(lqcd_slab *s, double mass, const double *in_dev, doubl
  * *iters and *true_residual are global (identical on every rank). */
 int lqcd_slab_cg_solve(lqcd_slab *s, double mass, double tol, int maxiter, const double *b_dev, double *x_dev,
                        int *iters, double *true_residual);
+/* The mixed-precision conjugate gradient of lqcd_cg_solve_mixed (fp32 iterations on fp32 copies of the links and
+ * of x, r, p, t; fp64 reliable updates; PAPER.md:151 ref. [2]) on the global system.
+ * The fp32 vectors travel as fp32 faces (sh*24 bytes per face), the x of a reliable update as fp64 faces; every
+ * inner product is combined in rank order, so the pause / resume / exit decisions are identical on every rank.
+ * One small launch per synchronisation point (no fused tails, no graph replay: the host loop has to see the
+ * pause).  Arguments and contract as lqcd_cg_solve_mixed; *iters, *reliable_updates, *true_residual are global. */
+int lqcd_slab_cg_solve_mixed(lqcd_slab *s, double mass, double tol, int maxiter, double delta, const double *b_dev,
+                             double *x_dev, int *iters, int *reliable_updates, double *true_residual);
 
 /* The same three operations on n slabs driven by the calling thread (n = nranks of every slab, slabs[r]
  * of rank r, all connected to each other).  in/out/b/x: arrays of n device pointers. */
@@ -119,6 +127,9 @@ int lqcd_slab_apply_MdagM_group(lqcd_slab *const *slabs, int n, double mass, con
                                 double *const *out_dev);
 int lqcd_slab_cg_solve_group(lqcd_slab *const *slabs, int n, double mass, double tol, int maxiter,
                              const double *const *b_dev, double *const *x_dev, int *iters, double *true_residual);
+int lqcd_slab_cg_solve_mixed_group(lqcd_slab *const *slabs, int n, double mass, double tol, int maxiter, double delta,
+                                   const double *const *b_dev, double *const *x_dev, int *iters, int *reliable_updates,
+                                   double *true_residual);
 
 /* CUDA IPC plumbing for one process per GPU: export the own mailbox as a 64-byte handle plus the
  * offset of the mailbox inside the allocation the handle names; open / close a peer's. */

@@ -32,6 +32,7 @@ struct lqcd_slab {
     size_t nvec;  // complex numbers per local vector
     // workspace (private) byte offsets
     size_t off_gauge, off_gghost, off_r, off_p, off_t, off_sc, off_ss, off_ticket, off_partials, off_hist, ws_needed;
+    size_t off_gauge_f, off_gghost_f, off_xf, off_rf, off_pf, off_tf;  // fp32 copies of the mixed-precision solver
     // mailbox (peer-visible) byte offsets
     size_t mb_word, mb_ghost, mb_needed;
     size_t max_blocks;
@@ -41,6 +42,7 @@ struct lqcd_slab {
     cudaStream_t stream;
     int device;
     bool memory_set, connected, gauge_loaded;
+    bool gauge_f_ready;  // the fp32 link copies match the loaded fp64 ones
     int recon, check_every, timeout_ms, use_graph, fuse_sync;
     unsigned long long seq;  // synchronisation points passed
     CgScalars* h_sc;         // pinned, 2 slots
@@ -55,6 +57,12 @@ struct lqcd_slab {
     cplx* r() const { return (cplx*)(ws + off_r); }
     cplx* p() const { return (cplx*)(ws + off_p); }
     cplx* t() const { return (cplx*)(ws + off_t); }
+    cplxf* gauge_f() const { return (cplxf*)(ws + off_gauge_f); }
+    cplxf* gghost_f() const { return (cplxf*)(ws + off_gghost_f); }
+    cplxf* xf() const { return (cplxf*)(ws + off_xf); }
+    cplxf* rf() const { return (cplxf*)(ws + off_rf); }
+    cplxf* pf() const { return (cplxf*)(ws + off_pf); }
+    cplxf* tf() const { return (cplxf*)(ws + off_tf); }
     CgScalars* sc() const { return (CgScalars*)(ws + off_sc); }
     SlabScalars* ss() const { return (SlabScalars*)(ws + off_ss); }
     double* hist() const { return (double*)(ws + off_hist); }
@@ -267,7 +275,7 @@ int launch_push_faces(lqcd_slab* s, const cplx* v)
     return LQCD_OK;
 }
 
-SlabSyncArgs sync_args(const lqcd_slab* s, int op, int nvals, double m2, double tol, int maxiter)
+SlabSyncArgs sync_args(const lqcd_slab* s, int op, int nvals, double m2, double tol, int maxiter, double delta = 0.0)
 {
     SlabSyncArgs a;
     memset(&a, 0, sizeof a);
@@ -283,6 +291,7 @@ SlabSyncArgs sync_args(const lqcd_slab* s, int op, int nvals, double m2, double 
     a.op = op;
     a.m2 = m2;
     a.tol = tol;
+    a.delta = delta;
     a.maxiter = maxiter;
     a.timeout_ns = (unsigned long long)s->timeout_ms * 1000000ull;
     return a;
@@ -294,7 +303,7 @@ SlabSyncArgs sync_args(const lqcd_slab* s, int op, int nvals, double m2, double 
 // in_producer: the producer kernel was launched with the synchronisation point in its last block
 // (fused(G)); only the host's count moves.
 int group_sync(const Group& G, int op, int nvals, double m2 = 0.0, double tol = 0.0, int maxiter = 0,
-               bool in_producer = false)
+               bool in_producer = false, double delta = 0.0)
 {
     for (int r = 0; r < G.n; ++r) G.s[r]->seq += 1;  // host copy: selects the ghost buffers; the kernels count on the device
     if (in_producer) return LQCD_OK;
@@ -302,7 +311,7 @@ int group_sync(const Group& G, int op, int nvals, double m2 = 0.0, double tol = 
         lqcd_slab* s = G.s[0];
         int rc = use_device(s);
         if (rc) return rc;
-        slab_signal_wait_combine_kernel<<<1, 32, 0, s->stream>>>(sync_args(s, op, nvals, m2, tol, maxiter));
+        slab_signal_wait_combine_kernel<<<1, 32, 0, s->stream>>>(sync_args(s, op, nvals, m2, tol, maxiter, delta));
         SLAB_LAUNCH_CHECK();
         return LQCD_OK;
     }
@@ -310,14 +319,14 @@ int group_sync(const Group& G, int op, int nvals, double m2 = 0.0, double tol = 
         lqcd_slab* s = G.s[r];
         int rc = use_device(s);
         if (rc) return rc;
-        slab_signal_kernel<<<1, 32, 0, s->stream>>>(sync_args(s, op, nvals, m2, tol, maxiter));
+        slab_signal_kernel<<<1, 32, 0, s->stream>>>(sync_args(s, op, nvals, m2, tol, maxiter, delta));
         SLAB_LAUNCH_CHECK();
     }
     for (int r = 0; r < G.n; ++r) {
         lqcd_slab* s = G.s[r];
         int rc = use_device(s);
         if (rc) return rc;
-        slab_wait_combine_kernel<<<1, 32, 0, s->stream>>>(sync_args(s, op, nvals, m2, tol, maxiter));
+        slab_wait_combine_kernel<<<1, 32, 0, s->stream>>>(sync_args(s, op, nvals, m2, tol, maxiter, delta));
         SLAB_LAUNCH_CHECK();
     }
     return LQCD_OK;
@@ -464,7 +473,7 @@ int group_iteration(const Group& G, double mass, cplx* const* x)
         lqcd_slab* s = G.s[r];
         rc = use_device(s);
         if (rc) return rc;
-        slab_cg_pupdate_kernel<kVecBlock><<<vec_grid(s), kVecBlock, 0, s->stream>>>(
+        slab_cg_pupdate_kernel<kVecBlock, cplx><<<vec_grid(s), kVecBlock, 0, s->stream>>>(
             s->r(), s->p(), vec_plan(s, vec_grid(s)), push_next(s), s->sc(), s->ss(), s->rs(), sync_args(s, SLAB_OP_PP, 1, 0.0, 0.0, 0), fz ? 1 : 0);
         SLAB_LAUNCH_CHECK();
     }
@@ -562,6 +571,18 @@ int group_cg(const Group& G, double mass, double tol, int maxiter, const cplx* c
     }
     rc = group_finish(G);
     if (rc) return rc;
+    // One counter again.  Inside the loop the host count selects the ghost buffers (it is baked into the launches, so
+    // it must advance with every enqueued iteration) and the device count tags the words (it must not be baked into a
+    // replayed graph); with the synchronisation point fused into the producers, iterations enqueued after convergence
+    // are complete no-ops, so the device count stops where the host count runs on.  Both are the same on every rank
+    // (the host loop is deterministic, the scalars bit-identical), which is all the protocol needs; and every ghost
+    // face has been consumed -- a rank passes the last real point only after its peers have signalled it, i.e. after
+    // their last Dslash.  From here on the host continues from the device's number (copied by group_finish).
+    for (int r = 0; r < G.n; ++r) {
+        if (G.s[r]->h_ss->seq > G.s[r]->seq) return fail(G.s[r], LQCD_ESTATE, "rank %d: device passed %llu synchronisation points, host enqueued %llu",
+                                                       r, G.s[r]->h_ss->seq, G.s[r]->seq);
+        G.s[r]->seq = G.s[r]->h_ss->seq;
+    }
 
     // S7: |b - A x| / |b| with a fresh A
     rc = group_first_hop(G, x);
@@ -588,6 +609,246 @@ int group_cg(const Group& G, double mass, double tol, int maxiter, const cplx* c
     *iters = h[0].iter;
     *true_residual = h[0].bb > 0.0 ? sqrt(h[0].res2 / h[0].bb) : 0.0;
     return h[0].rr_new <= h[0].thresh ? LQCD_OK : LQCD_MAXITER;
+}
+
+// ---------------------------------------------------------------- mixed precision on slabs (SURVEY.md 8(f) rows 3 + 4b)
+// The solver of lqcd_cg_solve_mixed (fp32 iterations, fp64 reliable updates) on the slab
+// decomposition: the fp32 vectors p and t travel as fp32 faces (half the NVLink bytes), the reliable update's x as
+// fp64 faces; every sum is combined in rank order as in the fp64 slab solver.  Separate launches per
+// synchronisation point (no fused tails, no graph replay): the host loop has to see `pause`.
+typedef StagArgs<cplxf> StagArgsF;
+
+SlabPushF push_next_f(const lqcd_slab* s)
+{
+    const SlabPush ph = push_next(s);
+    SlabPushF f;
+    f.lo = (cplxf*)ph.lo;  // the same ghost areas, read back as fp32 by the fp32 kernels
+    f.hi = (cplxf*)ph.hi;
+    f.sh = ph.sh;
+    f.Vh = ph.Vh;
+    return f;
+}
+
+StagArgsF stag_args_f(const lqcd_slab* s, int parity, const cplxf* in, cplxf* out, bool push)
+{
+    StagArgsF a;
+    memset(&a, 0, sizeof a);
+    a.g = s->g;
+    a.parity = parity;
+    a.gauge = s->gauge_f();
+    a.in = in;
+    a.out = out;
+    a.sc = s->sc();
+    a.rs = s->rs();
+    a.hist = s->hist();
+    a.sl.t0 = s->t0;
+    a.sl.L3g = s->L[3];
+    a.sl.sh = s->sh;
+    const int buf = (int)(s->seq & 1ull);
+    a.sl.ghost_lo = (const cplxf*)s->ghost(s->mb, buf, 0);
+    a.sl.ghost_hi = (const cplxf*)s->ghost(s->mb, buf, 1);
+    a.sl.gauge_ghost = s->gghost_f();
+    if (push) {
+        const SlabPushF ph = push_next_f(s);
+        a.sl.push_lo = ph.lo;
+        a.sl.push_hi = ph.hi;
+    }
+    a.sl.part = s->ss()->part;
+    return a;
+}
+
+template <int EPI>
+int launch_stag_f(lqcd_slab* s, const StagArgsF& a)
+{
+    const unsigned int grid = blocks_for(s->g.Vh, kStagBlock);
+    if (s->recon == 12)
+        stag_dslash_slab_kernel<EPI, kStagBlock, 12, cplxf><<<grid, kStagBlock, 0, s->stream>>>(a);
+    else
+        stag_dslash_slab_kernel<EPI, kStagBlock, 18, cplxf><<<grid, kStagBlock, 0, s->stream>>>(a);
+    SLAB_LAUNCH_CHECK();
+    return LQCD_OK;
+}
+
+int ensure_gauge_f(lqcd_slab* s)
+{
+    if (s->gauge_f_ready) return LQCD_OK;
+    const size_t nc = (size_t)(s->recon / 2);
+    gauge_narrow_kernel<<<148 * 8, 256, 0, s->stream>>>(s->gauge(), s->gauge_f(), (size_t)s->g.V * 4 * nc);
+    SLAB_LAUNCH_CHECK();
+    gauge_narrow_kernel<<<64, 256, 0, s->stream>>>(s->gghost(), s->gghost_f(), 2 * nc * (size_t)s->sh);
+    SLAB_LAUNCH_CHECK();
+    s->gauge_f_ready = true;
+    return LQCD_OK;
+}
+
+int group_pupdate_f(const Group& G)  // S5 on the fp32 copies; faces of ps -> neighbours
+{
+    for (int r = 0; r < G.n; ++r) {
+        lqcd_slab* s = G.s[r];
+        int rc = use_device(s);
+        if (rc) return rc;
+        slab_cg_pupdate_kernel<kVecBlock, cplxf><<<vec_grid(s), kVecBlock, 0, s->stream>>>(
+            s->rf(), s->pf(), vec_plan(s, vec_grid(s)), push_next_f(s), s->sc(), s->ss(), s->rs(), sync_args(s, SLAB_OP_PP, 1, 0.0, 0.0, 0), 0);
+        SLAB_LAUNCH_CHECK();
+    }
+    return group_sync(G, SLAB_OP_PP, 1);
+}
+
+int group_iteration_mixed(const Group& G, double mass)
+{
+    const double m2 = mass * mass;
+    int rc;
+    for (int r = 0; r < G.n; ++r) {  // S1: ts = D^_oe ps, partial <ts,ts>; fp32 faces of ts -> neighbours
+        lqcd_slab* s = G.s[r];
+        rc = use_device(s);
+        if (rc) return rc;
+        rc = launch_stag_f<SE_NORM>(s, stag_args_f(s, LQCD_ODD, s->pf(), s->tf(), true));
+        if (rc) return rc;
+    }
+    rc = group_sync(G, SLAB_OP_ALPHA, 1, m2);  // S2
+    if (rc) return rc;
+    for (int r = 0; r < G.n; ++r) {  // S3 on the fp32 vectors
+        lqcd_slab* s = G.s[r];
+        rc = use_device(s);
+        if (rc) return rc;
+        StagArgsF a = stag_args_f(s, LQCD_EVEN, s->tf(), nullptr, false);
+        a.m2 = m2;
+        a.p = s->pf();
+        a.x = s->xf();
+        a.r = s->rf();
+        rc = launch_stag_f<SE_CGUPDATE_MIXED>(s, a);
+        if (rc) return rc;
+    }
+    rc = group_sync(G, SLAB_OP_UPDATE_MIXED, 1);  // beta or pause, identically on every rank
+    if (rc) return rc;
+    return group_pupdate_f(G);
+}
+
+// The reliable update, all fp64: x += xs, xs = 0; r = b - A x with the faces of x and of D_oe x exchanged as in
+// the fp64 solver; rs = fl32(r); <r,r> combined over the ranks, beta, exit test; then the waiting fp32 p-update.
+int group_reliable_update(const Group& G, double mass, const cplx* const* b, cplx* const* x)
+{
+    int rc;
+    for (int r = 0; r < G.n; ++r) {
+        lqcd_slab* s = G.s[r];
+        rc = use_device(s);
+        if (rc) return rc;
+        mixed_accumulate_kernel<kVecBlock><<<vec_grid(s), kVecBlock, 0, s->stream>>>(x[r], s->xf(), s->nvec, s->sc(), 1);
+        SLAB_LAUNCH_CHECK();
+    }
+    rc = group_first_hop(G, x);  // faces of x, t = D_oe x, faces of t
+    if (rc) return rc;
+    for (int r = 0; r < G.n; ++r) {
+        lqcd_slab* s = G.s[r];
+        rc = use_device(s);
+        if (rc) return rc;
+        StagArgsD a = stag_args(s, LQCD_EVEN, s->t(), nullptr, false);
+        a.m2 = mass * mass;
+        a.p = x[r];
+        a.b = b[r];
+        a.rf = s->rf();
+        rc = launch_stag<SE_RELIABLE>(s, a);
+        if (rc) return rc;
+    }
+    rc = group_sync(G, SLAB_OP_RELIABLE, 1);
+    if (rc) return rc;
+    return group_pupdate_f(G);
+}
+
+int group_cg_mixed(const Group& G, double mass, double tol, double delta, int maxiter, const cplx* const* b, cplx* const* x,
+                   int* iters, int* reliable_updates, double* true_residual)
+{
+    int rc;
+    lqcd_slab* s0 = G.s[0];
+    for (int r = 0; r < G.n; ++r) {
+        lqcd_slab* s = G.s[r];
+        rc = use_device(s);
+        if (rc) return rc;
+        rc = ensure_gauge_f(s);
+        if (rc) return rc;
+        slab_cg_init_mixed_kernel<kVecBlock><<<vec_grid(s), kVecBlock, 0, s->stream>>>(
+            b[r], x[r], s->xf(), s->rf(), s->pf(), vec_plan(s, vec_grid(s)), push_next_f(s), s->ss(), s->rs());
+        SLAB_LAUNCH_CHECK();
+    }
+    rc = group_sync(G, SLAB_OP_INIT_MIXED, 2, 0.0, tol, maxiter, false, delta);
+    if (rc) return rc;
+
+    // Host loop as cg_run_mixed of lqcd_api.cu: batches of iterations enqueued while the previous batch's scalars
+    // travel; iterations enqueued after the device paused (or finished) are no-ops on every rank -- the
+    // synchronisation kernels still run, so the ranks stay in step -- and the update sequence is enqueued exactly
+    // once per pause.  The scalars are bit-identical on all ranks; rank 0's copy (of this process) is read.
+    CgScalars* h = s0->h_sc;
+    const int batch = s0->check_every;
+    int slot = 0, updates_enqueued = 0;
+    bool pending[2] = { false, false };
+    bool finished = maxiter <= 0;
+    while (!finished) {
+        for (int k = 0; k < batch; ++k) {
+            rc = group_iteration_mixed(G, mass);
+            if (rc) return rc;
+        }
+        rc = use_device(s0);
+        if (rc) return rc;
+        rc = read_scalars(s0, slot);
+        if (rc) return rc;
+        pending[slot] = true;
+        const int look = slot ^ 1;
+        if (pending[look]) {
+            lqcd_slab* s = s0;
+            SLAB_CUDA(cudaEventSynchronize(s->ev[look]));
+            pending[look] = false;
+            if (h[look].done) {
+                finished = true;
+            } else if (h[look].pause && h[look].nupd == updates_enqueued) {
+                rc = group_reliable_update(G, mass, b, x);
+                if (rc) return rc;
+                ++updates_enqueued;
+            }
+        }
+        slot ^= 1;
+    }
+    for (int r = 0; r < G.n; ++r) {  // whatever the fp32 iteration still holds goes into x
+        lqcd_slab* s = G.s[r];
+        rc = use_device(s);
+        if (rc) return rc;
+        mixed_accumulate_kernel<kVecBlock><<<vec_grid(s), kVecBlock, 0, s->stream>>>(x[r], s->xf(), s->nvec, s->sc(), 0);
+        SLAB_LAUNCH_CHECK();
+    }
+    rc = use_device(s0);
+    if (rc) return rc;
+    rc = read_scalars(s0, 0);
+    if (rc) return rc;
+    rc = group_finish(G);
+    if (rc) return rc;
+    const int it = h[0].iter, nupd = h[0].nupd;
+    const bool converged = h[0].bb == 0.0 || (h[0].rr_new <= h[0].thresh && !h[0].pause && nupd > 0);
+
+    // S7: |b - A x| / |b| with a fresh fp64 A
+    rc = group_first_hop(G, x);
+    if (rc) return rc;
+    for (int r = 0; r < G.n; ++r) {
+        lqcd_slab* s = G.s[r];
+        rc = use_device(s);
+        if (rc) return rc;
+        StagArgsD a = stag_args(s, LQCD_EVEN, s->t(), nullptr, false);
+        a.m2 = mass * mass;
+        a.p = x[r];
+        a.b = b[r];
+        rc = launch_stag<SE_RESIDUAL>(s, a);
+        if (rc) return rc;
+    }
+    rc = group_sync(G, SLAB_OP_RES2, 1);
+    if (rc) return rc;
+    rc = use_device(s0);
+    if (rc) return rc;
+    rc = read_scalars(s0, 0);
+    if (rc) return rc;
+    rc = group_finish(G);
+    if (rc) return rc;
+    *iters = it;
+    *reliable_updates = nupd;
+    *true_residual = h[0].bb > 0.0 ? sqrt(h[0].res2 / h[0].bb) : 0.0;
+    return converged ? LQCD_OK : LQCD_MAXITER;
 }
 
 }  // namespace
@@ -645,6 +906,13 @@ int lqcd_slab_create(lqcd_slab** out, int L0, int L1, int L2, int L3, int rank, 
     c->off_ticket = off;    off += kAlign;
     c->off_partials = off;  off += align_up(c->max_blocks * sizeof(double));
     c->off_hist = off;      off += align_up((size_t)kHistCap * sizeof(double));
+    const size_t vecf_bytes = align_up(c->nvec * sizeof(cplxf));
+    c->off_gauge_f = off;   off += align_up((size_t)V * 36 * sizeof(cplxf));
+    c->off_gghost_f = off;  off += align_up(2 * 9 * (size_t)c->sh * sizeof(cplxf));
+    c->off_xf = off;        off += vecf_bytes;
+    c->off_rf = off;        off += vecf_bytes;
+    c->off_pf = off;        off += vecf_bytes;
+    c->off_tf = off;        off += vecf_bytes;
     c->ws_needed = off;
 
     off = 0;
@@ -698,6 +966,7 @@ int lqcd_slab_set_memory(lqcd_slab* s, void* workspace_dev, size_t workspace_byt
     s->memory_set = true;
     s->connected = false;
     s->gauge_loaded = false;
+    s->gauge_f_ready = false;
     s->seq = 0;
     SLAB_CUDA(cudaMemsetAsync(s->ws + s->off_sc, 0, align_up(sizeof(CgScalars)) + align_up(sizeof(SlabScalars)) + kAlign, s->stream));
     SLAB_CUDA(cudaMemsetAsync(s->mb, 0, s->mb_ghost, s->stream));  // the tagged words (tag 0 = no synchronisation point)
@@ -723,7 +992,7 @@ int lqcd_slab_set_option(lqcd_slab* s, int option, int value)
     if (!s) return LQCD_EARG;
     if (option == LQCD_SLAB_OPT_RECONSTRUCT) {
         if (value != 18 && value != 12) return fail(s, LQCD_EARG, "reconstruct must be 18 or 12");
-        if (value != s->recon) s->gauge_loaded = false;
+        if (value != s->recon) s->gauge_loaded = s->gauge_f_ready = false;
         s->recon = value;
         return LQCD_OK;
     }
@@ -763,15 +1032,16 @@ int lqcd_slab_load_gauge(lqcd_slab* s, const double* u_local_dev, const double* 
         gauge_reorder_kernel<256, kReorderTile, 12, cplx><<<grid, 256, 0, s->stream>>>((const cplx*)u_local_dev, s->gauge(),
                                                                                        (size_t)s->g.Vh);
         SLAB_LAUNCH_CHECK();
-        slab_ghost_links_kernel<12><<<ggrid, 256, 0, s->stream>>>((const cplx*)u3_below_dev, s->gghost(), (size_t)s->sh);
+        slab_ghost_links_kernel<12, cplx><<<ggrid, 256, 0, s->stream>>>((const cplx*)u3_below_dev, s->gghost(), (size_t)s->sh);
     } else {
         gauge_reorder_kernel<256, kReorderTile, 18, cplx><<<grid, 256, 0, s->stream>>>((const cplx*)u_local_dev, s->gauge(),
                                                                                        (size_t)s->g.Vh);
         SLAB_LAUNCH_CHECK();
-        slab_ghost_links_kernel<18><<<ggrid, 256, 0, s->stream>>>((const cplx*)u3_below_dev, s->gghost(), (size_t)s->sh);
+        slab_ghost_links_kernel<18, cplx><<<ggrid, 256, 0, s->stream>>>((const cplx*)u3_below_dev, s->gghost(), (size_t)s->sh);
     }
     SLAB_LAUNCH_CHECK();
     s->gauge_loaded = true;
+    s->gauge_f_ready = false;
     return LQCD_OK;
 }
 
@@ -853,6 +1123,39 @@ int lqcd_slab_cg_solve(lqcd_slab* s, double mass, double tol, int maxiter, const
     const cplx* b[1] = { (const cplx*)b_dev };
     cplx* x[1] = { (cplx*)x_dev };
     return group_cg(G, mass, tol, maxiter, b, x, iters, true_residual);
+}
+
+int lqcd_slab_cg_solve_mixed_group(lqcd_slab* const* slabs, int n, double mass, double tol, int maxiter, double delta,
+                                   const double* const* b_dev, double* const* x_dev, int* iters, int* reliable_updates,
+                                   double* true_residual)
+{
+    const Group G = { slabs, n };
+    int rc = group_check(G, true);
+    if (rc) return rc;
+    lqcd_slab* s = slabs[0];
+    if (!b_dev || !x_dev || !iters || !reliable_updates || !true_residual) return fail(s, LQCD_EARG, "null pointer argument");
+    if (!(tol >= 0.0) || maxiter < 0) return fail(s, LQCD_EARG, "tol must be >= 0 and maxiter >= 0");
+    if (!(delta > 0.0 && delta < 1.0)) return fail(s, LQCD_EARG, "delta must be in (0,1)");
+    for (int r = 0; r < n; ++r)
+        if (!b_dev[r] || !x_dev[r] || b_dev[r] == x_dev[r]) return fail(s, LQCD_EARG, "null or aliased vector of rank %d", r);
+    return group_cg_mixed(G, mass, tol, delta, maxiter, (const cplx* const*)b_dev, (cplx* const*)x_dev, iters, reliable_updates,
+                          true_residual);
+}
+
+int lqcd_slab_cg_solve_mixed(lqcd_slab* s, double mass, double tol, int maxiter, double delta, const double* b_dev, double* x_dev,
+                             int* iters, int* reliable_updates, double* true_residual)
+{
+    int rc = single_check(s, true);
+    if (rc) return rc;
+    if (!b_dev || !x_dev || !iters || !reliable_updates || !true_residual || b_dev == x_dev)
+        return fail(s, LQCD_EARG, "null or aliased argument");
+    if (!(tol >= 0.0) || maxiter < 0) return fail(s, LQCD_EARG, "tol must be >= 0 and maxiter >= 0");
+    if (!(delta > 0.0 && delta < 1.0)) return fail(s, LQCD_EARG, "delta must be in (0,1)");
+    lqcd_slab* one[1] = { s };
+    const Group G = { one, 1 };
+    const cplx* b[1] = { (const cplx*)b_dev };
+    cplx* x[1] = { (cplx*)x_dev };
+    return group_cg_mixed(G, mass, tol, delta, maxiter, b, x, iters, reliable_updates, true_residual);
 }
 
 // ---- CUDA IPC: mailboxes across processes

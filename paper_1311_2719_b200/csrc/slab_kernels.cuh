@@ -39,12 +39,15 @@ static __global__ void slab_signal_wait_combine_kernel(const SlabSyncArgs a) { s
 
 // Where the two boundary time-slices of a slab vector go: element (c, e) of local slice 0 into the
 // lower neighbour's ghost_hi, of local slice T-1 into the upper neighbour's ghost_lo.
-struct SlabPush {
-    cplx* lo;
-    cplx* hi;
+template <class C>
+struct SlabPushT {
+    C* lo;
+    C* hi;
     int sh;       // sites of one parity in a time-slice
     int Vh;       // local sites of one parity
 };
+typedef SlabPushT<cplx> SlabPush;    // fp64 vectors
+typedef SlabPushT<cplxf> SlabPushF;  // fp32 vectors of the mixed-precision solver (the same ghost areas, half used)
 
 // The vector kernels walk the n = 3 Vh elements in a FACE-FIRST order: virtual index v < 6 sh is an element of one
 // of the two boundary time-slices (face f = v / sh: colour f / 2, first or last slice), the rest is the interior.
@@ -79,7 +82,8 @@ __device__ __forceinline__ void slab_vec_range(const SlabVecPlan& pl, size_t& v0
 }
 
 // virtual index -> element index i = c Vh + e, and where (if anywhere) the element goes in the neighbours' ghosts
-__device__ __forceinline__ size_t slab_vec_elem(const SlabPush& ph, const SlabVecPlan& pl, size_t v, cplx*& peer_dst)
+template <class C>
+__device__ __forceinline__ size_t slab_vec_elem(const SlabPushT<C>& ph, const SlabVecPlan& pl, size_t v, C*& peer_dst)
 {
     const size_t sh = (size_t)ph.sh, Vh = (size_t)ph.Vh;
     peer_dst = nullptr;
@@ -149,31 +153,34 @@ __global__ void __launch_bounds__(BLOCK) slab_cg_init_kernel(const cplx* __restr
         grid_sum<BLOCK>(local, rs, [ss](double bb) { ss->part[0] = bb; });
 }
 
-// S5 on a slab: p = r + beta p, partial <p,p>; the faces of the new p go to the neighbours.
-template <int BLOCK>
-__global__ void __launch_bounds__(BLOCK) slab_cg_pupdate_kernel(const cplx* __restrict__ r, cplx* __restrict__ p, SlabVecPlan pl,
-                                                                SlabPush ph, const CgScalars* sc, SlabScalars* ss,
+// S5 on a slab: p = r + beta p, partial <p,p>; the faces of the new p go to the neighbours.  C = cplx, or cplxf for
+// the fp32 inner iteration of the mixed-precision solver (evaluated in fp64, rounded on store, the norm taken of
+// the stored value: as cg_pupdate_kernel).
+template <int BLOCK, class C>
+__global__ void __launch_bounds__(BLOCK) slab_cg_pupdate_kernel(const C* __restrict__ r, C* __restrict__ p, SlabVecPlan pl,
+                                                                SlabPushT<C> ph, const CgScalars* sc, SlabScalars* ss,
                                                                 ReduceScratch rs, const SlabSyncArgs sy, int fused)
 {
-    if (sc->done) return;
+    if (sc->done | sc->pause) return;
     const double beta = sc->beta;
     double local = 0.0;
     bool wrote_peer = false;
     size_t v0, v1;
     slab_vec_range(pl, v0, v1);
     for (size_t v = v0 + threadIdx.x; v < v1; v += BLOCK) {
-        cplx* dst;
+        C* dst;
         const size_t i = slab_vec_elem(ph, pl, v, dst);
-        const cplx rv = r[i];
-        cplx pv = p[i];
+        const double2 rv = to_d(r[i]);
+        double2 pv = to_d(p[i]);
         pv.x = fma(beta, pv.x, rv.x);
         pv.y = fma(beta, pv.y, rv.y);
-        p[i] = pv;
+        const C ps = to_cplx(pv, (C*)0);
+        p[i] = ps;
         if (dst) {
-            *dst = pv;
+            *dst = ps;
             wrote_peer = true;
         }
-        local += cnorm2(pv);
+        local += cnorm2(ps);
     }
     if (fused)
         grid_sum_block<BLOCK>(local, wrote_peer, rs, [&sy](double pp) { slab_sync_tail<BLOCK>(sy, pp); });
@@ -181,9 +188,39 @@ __global__ void __launch_bounds__(BLOCK) slab_cg_pupdate_kernel(const cplx* __re
         grid_sum<BLOCK>(local, rs, [ss](double pp) { ss->part[0] = pp; });
 }
 
+// S6 of the mixed-precision solver on a slab (cg_init_mixed_kernel): x = 0 (fp64), xs = 0, rs = ps = fl32(b), partial
+// <b,b> from the fp64 source and <ps,ps> from its fp32 copy; the faces of ps go to the neighbours.
+template <int BLOCK>
+__global__ void __launch_bounds__(BLOCK) slab_cg_init_mixed_kernel(const cplx* __restrict__ b, cplx* __restrict__ x,
+                                                                   cplxf* __restrict__ xs, cplxf* __restrict__ rs_,
+                                                                   cplxf* __restrict__ ps, SlabVecPlan pl, SlabPushF ph,
+                                                                   SlabScalars* ss, ReduceScratch rs)
+{
+    double local[2] = { 0.0, 0.0 };
+    size_t v0, v1;
+    slab_vec_range(pl, v0, v1);
+    for (size_t v = v0 + threadIdx.x; v < v1; v += BLOCK) {
+        cplxf* dst;
+        const size_t i = slab_vec_elem(ph, pl, v, dst);
+        const cplx val = b[i];
+        const cplxf vf = make_float2((float)val.x, (float)val.y);
+        x[i] = cmake(0.0, 0.0);
+        xs[i] = make_float2(0.f, 0.f);
+        rs_[i] = vf;
+        ps[i] = vf;
+        if (dst) *dst = vf;
+        local[0] += cnorm2(val);
+        local[1] += cnorm2(vf);
+    }
+    grid_sum_n<BLOCK, 2>(local, rs, [ss](const double (&tot)[2]) {
+        ss->part[0] = tot[0];
+        ss->part[1] = tot[1];
+    });
+}
+
 // U_3 of the time-slice below the slab: canonical [parity][sh][3][3] -> [parity][NC][sh].
-template <int RECON>
-__global__ void slab_ghost_links_kernel(const cplx* __restrict__ u3, cplx* __restrict__ soa, size_t sh)
+template <int RECON, class C>
+__global__ void slab_ghost_links_kernel(const cplx* __restrict__ u3, C* __restrict__ soa, size_t sh)
 {
     constexpr int NC = RECON / 2;
     const size_t n = 2 * sh * NC;
@@ -191,7 +228,7 @@ __global__ void slab_ghost_links_kernel(const cplx* __restrict__ u3, cplx* __res
         const size_t parity = i / (sh * NC);
         const size_t rest = i - parity * sh * NC;
         const size_t k = rest / sh, f = rest - k * sh;
-        soa[i] = u3[(parity * sh + f) * 9 + k];
+        soa[i] = to_cplx(u3[(parity * sh + f) * 9 + k], (C*)0);
     }
 }
 

@@ -39,7 +39,11 @@ enum SlabOp {
     SLAB_OP_ALPHA = 2,   // total = <t,t>: alpha = rr / (m^2 pp + tt)
     SLAB_OP_UPDATE = 3,  // total = <r,r> after the update: beta, exit test
     SLAB_OP_PP = 4,      // total = <p,p>
-    SLAB_OP_RES2 = 5     // total = |b - A x|^2
+    SLAB_OP_RES2 = 5,    // total = |b - A x|^2
+    // mixed-precision solver on slabs (SURVEY.md 8(f) rows 3 + 4b; the scalar steps of reduce.cuh)
+    SLAB_OP_INIT_MIXED = 6,    // totals = <b,b> (fp64 source), <ps,ps> (its fp32 copy)
+    SLAB_OP_UPDATE_MIXED = 7,  // total = <rs,rs> after the fp32 update: may pause for a reliable update
+    SLAB_OP_RELIABLE = 8       // total = <r,r> of the fp64 residual: resumes the paused iteration
 };
 
 struct SlabSyncArgs {
@@ -51,7 +55,7 @@ struct SlabSyncArgs {
     CgScalars* sc;
     double* hist;
     int op;
-    double m2, tol;
+    double m2, tol, delta;
     int maxiter;
     unsigned long long timeout_ns;
 };
@@ -145,8 +149,29 @@ __device__ __forceinline__ void slab_combine(const SlabSyncArgs& a, unsigned lon
         a.hist[0] = bb;
         break;
     }
+    case SLAB_OP_INIT_MIXED: {
+        const double bb = total[0];
+        sc->rr = bb;
+        sc->rr_new = bb;
+        sc->bb = bb;
+        sc->pp = total[1];
+        sc->tt = 0.0;
+        sc->alpha = 0.0;
+        sc->beta = 0.0;
+        sc->thresh = a.tol * a.tol * bb;
+        sc->res2 = 0.0;
+        sc->rmax = sqrt(bb);
+        sc->delta = a.delta;
+        sc->iter = 0;
+        sc->maxiter = a.maxiter;
+        sc->done = (bb == 0.0 || a.maxiter <= 0) ? 1 : 0;
+        sc->pause = 0;
+        sc->nupd = 0;
+        a.hist[0] = bb;
+        break;
+    }
     case SLAB_OP_ALPHA:
-        if (sc->done) break;  // the producer was a no-op: `part` is stale
+        if (sc->done | sc->pause) break;  // the producer was a no-op: `part` is stale
         sc->tt = total[0];
         sc->alpha = sc->rr / (a.m2 * sc->pp + total[0]);
         break;
@@ -154,8 +179,15 @@ __device__ __forceinline__ void slab_combine(const SlabSyncArgs& a, unsigned lon
         if (sc->done) break;
         cg_after_update(sc, a.hist, total[0]);
         break;
+    case SLAB_OP_UPDATE_MIXED:
+        if (sc->done | sc->pause) break;
+        cg_after_update_mixed(sc, a.hist, total[0]);
+        break;
+    case SLAB_OP_RELIABLE:
+        cg_after_reliable(sc, a.hist, total[0]);
+        break;
     case SLAB_OP_PP:
-        if (sc->done) break;
+        if (sc->done | sc->pause) break;
         sc->pp = total[0];
         break;
     case SLAB_OP_RES2:

@@ -223,7 +223,16 @@ __device__ __forceinline__ void stag_dslash_body(const StagArgs<C>& a, const Sla
                     st_vec(a.out + c * Vh + e, acc[c]);
                     local += cnorm2(acc[c]);
                 }
-            } else if (EPI == SE_CGUPDATE) {
+            } else if (EPI == SE_RELIABLE) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const size_t i = c * Vh + e;
+                    const double2 xv = to_d(a.p[i]), bv = to_d(a.b[i]), q = to_d(acc[c]);
+                    const double2 rv = cmake(bv.x - fma(a.m2, xv.x, -q.x), bv.y - fma(a.m2, xv.y, -q.y));
+                    a.rf[i] = make_float2((float)rv.x, (float)rv.y);
+                    local += cnorm2(rv);
+                }
+            } else if (EPI == SE_CGUPDATE || EPI == SE_CGUPDATE_MIXED) {
                 const double alpha = a.sc->alpha;
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {

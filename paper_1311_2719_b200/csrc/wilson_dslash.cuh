@@ -114,8 +114,12 @@ __device__ __forceinline__ void wilson_hop_math(const cplx U[9], const cplx psi[
     }
 }
 
-template <int MU, bool PLUS, bool ADJ, int RECON, int LINKS>
-__device__ __forceinline__ void wilson_hop(const cplx* __restrict__ link, size_t Vh, const cplx* __restrict__ src,
+// VL: how the spinor is loaded (device_common.cuh).  The one-parity kernels are also launched with in == out
+// (the even-odd solver keeps an intermediate in the other half of the same array: reads go to one parity, writes
+// to the other, never to a shared 128-byte line) -- legal for ordinary loads, not for the read-only path, whose
+// contract is that the kernel writes nothing it reads through it: they take VL_PLAIN and no __restrict__.
+template <int MU, bool PLUS, bool ADJ, int RECON, int LINKS, int VL>
+__device__ __forceinline__ void wilson_hop(const cplx* __restrict__ link, size_t Vh, const cplx* src,
                                            size_t V, double sign, cplx acc[4][3])
 {
     cplx U[9], psi[4][3];
@@ -123,12 +127,12 @@ __device__ __forceinline__ void wilson_hop(const cplx* __restrict__ link, size_t
 #pragma unroll
     for (int s = 0; s < 4; ++s)
 #pragma unroll
-        for (int c = 0; c < 3; ++c) psi[s][c] = ld_keep(src + (size_t)(s * 3 + c) * V);
+        for (int c = 0; c < 3; ++c) psi[s][c] = ld_vec<VL>(src + (size_t)(s * 3 + c) * V);
     reconstruct_link<RECON>(U);
     wilson_hop_math<MU, PLUS, ADJ>(U, psi, sign, acc);
 }
 
-template <int MU, bool DAGGER, int RECON, int LINKS>
+template <int MU, bool DAGGER, int RECON, int LINKS, int VL>
 __device__ __forceinline__ void wilson_dir(const WilsonArgs& a, const Site& s, int parity, cplx acc[4][3])
 {
     const size_t Vh = (size_t)a.g.Vh, V = (size_t)a.g.V;
@@ -138,8 +142,8 @@ __device__ __forceinline__ void wilson_dir(const WilsonArgs& a, const Site& s, i
     const cplx* Uf = a.gauge + (size_t)((parity * 4 + MU) * (RECON / 2)) * Vh + s.e;
     const cplx* Ub = a.gauge + (size_t)(((1 - parity) * 4 + MU) * (RECON / 2)) * Vh + eb;
     // D: forward (1-gamma), backward (1+gamma);  D^+: forward (1+gamma), backward (1-gamma)
-    wilson_hop<MU, DAGGER, false, RECON, LINKS>(Uf, Vh, a.in + other + ef, V, bc_fwd<MU>(a.g, s), acc);
-    wilson_hop<MU, !DAGGER, true, RECON, LINKS>(Ub, Vh, a.in + other + eb, V, bc_bwd<MU>(a.g, s), acc);
+    wilson_hop<MU, DAGGER, false, RECON, LINKS, VL>(Uf, Vh, a.in + other + ef, V, bc_fwd<MU>(a.g, s), acc);
+    wilson_hop<MU, !DAGGER, true, RECON, LINKS, VL>(Ub, Vh, a.in + other + eb, V, bc_bwd<MU>(a.g, s), acc);
 }
 
 // Which site a thread owns.  One-parity kernels cover the Vh sites of a.parity.  The full-lattice kernels
@@ -348,12 +352,13 @@ __global__ void __launch_bounds__(BLOCK, LQCD_WILSON_MINB) wilson_dslash_kernel(
         }
     }
 #endif
+    constexpr int VL = wilson_one_parity(EPI) ? VL_PLAIN : VL_NC;
     if (active) {
         const Site st = decode_site(a.g, parity, e);
-        wilson_dir<0, DAGGER, RECON, LINKS>(a, st, parity, acc);
-        wilson_dir<1, DAGGER, RECON, LINKS>(a, st, parity, acc);
-        wilson_dir<2, DAGGER, RECON, LINKS>(a, st, parity, acc);
-        wilson_dir<3, DAGGER, RECON, LINKS>(a, st, parity, acc);
+        wilson_dir<0, DAGGER, RECON, LINKS, VL>(a, st, parity, acc);
+        wilson_dir<1, DAGGER, RECON, LINKS, VL>(a, st, parity, acc);
+        wilson_dir<2, DAGGER, RECON, LINKS, VL>(a, st, parity, acc);
+        wilson_dir<3, DAGGER, RECON, LINKS, VL>(a, st, parity, acc);
     }
     wilson_epilogue<EPI, BLOCK>(a, active, gsite, acc);
 }

@@ -138,6 +138,9 @@ def _lib():
         L.lqcd_slab_dslash.argtypes = [P, I, P, P]
         L.lqcd_slab_apply_MdagM.argtypes = [P, D, P, P]
         L.lqcd_slab_cg_solve.argtypes = [P, D, D, I, P, P, ctypes.POINTER(I), ctypes.POINTER(D)]
+        L.lqcd_slab_cg_solve_mixed.argtypes = [P, D, D, I, D, P, P, ctypes.POINTER(I), ctypes.POINTER(I), ctypes.POINTER(D)]
+        L.lqcd_slab_cg_solve_mixed_group.argtypes = [PP, I, D, D, I, D, PP, PP, ctypes.POINTER(I), ctypes.POINTER(I),
+                                                     ctypes.POINTER(D)]
         L.lqcd_slab_dslash_group.argtypes = [PP, I, I, PP, PP]
         L.lqcd_slab_apply_MdagM_group.argtypes = [PP, I, D, PP, PP]
         L.lqcd_slab_cg_solve_group.argtypes = [PP, I, D, D, I, PP, PP, ctypes.POINTER(I), ctypes.POINTER(D)]
@@ -264,6 +267,14 @@ class Slab:
                                                       self._vec(x), ctypes.byref(it), ctypes.byref(res)))
         return x, it.value, res.value, rc
 
+    def cg_solve_mixed(self, mass: float, tol: float, maxiter: int, b, x, delta: float = 0.1):
+        it, nu, res = ctypes.c_int(), ctypes.c_int(), ctypes.c_double()
+        self.stream.wait_stream(torch.cuda.current_stream(self.device))
+        rc = self._check(self._lib.lqcd_slab_cg_solve_mixed(self._s, float(mass), float(tol), int(maxiter), float(delta),
+                                                            self._vec(b), self._vec(x), ctypes.byref(it), ctypes.byref(nu),
+                                                            ctypes.byref(res)))
+        return x, it.value, nu.value, res.value, rc
+
     def sync_points(self) -> int:
         return int(self._lib.lqcd_slab_sync_points(self._s))
 
@@ -355,6 +366,14 @@ class SlabGroup:
         rc = self._check(self._lib.lqcd_slab_cg_solve_group(self._arr, self.nranks, float(mass), float(tol), int(maxiter),
                                                             self._ptrs(b), self._ptrs(x), ctypes.byref(it), ctypes.byref(res)))
         return x, it.value, res.value, rc
+
+    def cg_solve_mixed(self, mass: float, tol: float, maxiter: int, b, x, delta: float = 0.1):
+        it, nu, res = ctypes.c_int(), ctypes.c_int(), ctypes.c_double()
+        self._pre()
+        rc = self._check(self._lib.lqcd_slab_cg_solve_mixed_group(self._arr, self.nranks, float(mass), float(tol), int(maxiter),
+                                                                  float(delta), self._ptrs(b), self._ptrs(x), ctypes.byref(it),
+                                                                  ctypes.byref(nu), ctypes.byref(res)))
+        return x, it.value, nu.value, res.value, rc
 
     def synchronize(self):
         for s in self.slabs:

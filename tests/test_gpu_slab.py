@@ -327,6 +327,97 @@ def test_slab_cg_cfg5_eight_slabs(sl, cfg5_inputs):
     check_sampled_solution(x, ref, CG_TOL)
 
 
+# ------------------------------------------------------------------ mixed precision on slabs (SURVEY.md 8(f) rows 3 + 4b)
+def _count_close(a, b):
+    return abs(a - b) <= max(3, 0.03 * b)
+
+
+@pytest.mark.parametrize("recon", [18, 12])
+@pytest.mark.parametrize("dims,kind,mass,nranks", [((4, 4, 4, 4), "random_su3", 0.1, 1), ((4, 4, 4, 4), "random_su3", 0.1, 2),
+                                                   ((6, 4, 2, 12), "smooth", 0.05, 3), ((8, 8, 8, 8), "haar", 0.03, 2),
+                                                   ((8, 8, 8, 8), "haar", 0.03, 4), ((16, 16, 16, 16), "smooth", 0.05, 4),
+                                                   ((16, 16, 16, 16), "smooth", 0.05, 8)])
+def test_slab_mixed_cg_matches_global_mixed_oracle(sl, dims, kind, mass, nranks, recon):
+    """lqcd_slab_cg_solve_mixed_group against the oracle's mixed-precision CG and its fp64 CG on the UNDIVIDED lattice,
+    under the contract of tests/test_gpu_mixed.py: exit declared on an fp64 residual (true residual
+    <= tol), solution within the bound two tol-converged solutions obey (and 1e-8), iteration / update counts within
+    a few per cent / +-2 (fp32 rounding and the grouping of the sums perturb the trajectory), first residuals to
+    fp32 accuracy."""
+    tol = 1e-10
+    u = synth.gauge_field(dims, kind, 111)
+    b = synth.source(dims, "staggered", 112)
+    want = oracle.cg_mixed(dims, u, mass, tol, 20000, b, history=True)
+    plain = oracle.cg(dims, 0, u, mass, tol, 20000, b)
+    assert want["status"] == 0
+    g = group_for(sl, dims, nranks, u, recon)
+    try:
+        g.set_option(sl.OPT_CHECK_EVERY, 4)
+        xs, it, nupd, res, status = g.cg_solve_mixed(mass, tol, 20000, g.scatter(torch.from_numpy(b)), g.new_vectors())
+        x = gathered(sl, xs)
+    finally:
+        g.close()
+    assert status == 0 and res <= tol
+    bound = 2 * tol * np.linalg.norm(b) / mass ** 2
+    assert np.linalg.norm(x - plain["x"]) <= min(bound, 1e-8 * np.linalg.norm(plain["x"]))
+    assert np.linalg.norm(x - want["x"]) <= min(bound, 1e-8 * np.linalg.norm(want["x"]))
+    assert _count_close(it, want["iters"]) and abs(nupd - want["updates"]) <= 2
+    true = rel(oracle.apply_MdagM(dims, 0, u, mass, x), b)
+    assert abs(true - res) <= 1e-3 * true + 1e-15
+
+
+def test_slab_mixed_cg_agrees_with_the_single_gpu_mixed_solver_and_batching(sl):
+    """The decomposition and the batch size must not change the mixed solver: counts as the undivided solver's, the
+    same solution to far below the contract, bit-identical results whatever check_every, edge cases."""
+    from paper_1311_2719_b200 import lqcd
+    c, u, b = synth.config_inputs(2)
+    with lqcd.Lattice(c["dims"], lqcd.STAGGERED) as lat:
+        lat.load_gauge(torch.from_numpy(u).cuda())
+        x1, it1, n1, res1, st1 = lat.cg_solve_mixed(c["param"], c["tol"], 20000, torch.from_numpy(b).cuda())
+        x1 = x1.cpu().numpy()
+    g = group_for(sl, c["dims"], 4, u)
+    try:
+        got = []
+        for every in (1, 8):
+            g.set_option(sl.OPT_CHECK_EVERY, every)
+            xs, it, nupd, res, status = g.cg_solve_mixed(c["param"], c["tol"], 20000, g.scatter(torch.from_numpy(b)), g.new_vectors())
+            got.append((gathered(sl, xs), it, nupd, res, status))
+        assert got[0][1:] == got[1][1:] and np.array_equal(got[0][0], got[1][0])
+        x, it, nupd, res, status = got[0]
+        assert status == st1 == 0 and _count_close(it, it1) and abs(nupd - n1) <= 2 and res <= c["tol"]
+        assert rel(x, x1) <= 1e-8
+        # b = 0, maxiter = 0, a fixed number of iterations (tol = 0)
+        zero = [torch.zeros_like(v) for v in g.scatter(torch.from_numpy(b))]
+        xs, it, nupd, res, status = g.cg_solve_mixed(c["param"], c["tol"], 100, zero, g.new_vectors())
+        assert it == 0 and res == 0.0 and status == 0 and not gathered(sl, xs).any()
+        xs, it, nupd, res, status = g.cg_solve_mixed(c["param"], c["tol"], 0, g.scatter(torch.from_numpy(b)), g.new_vectors())
+        assert it == 0 and status == 1 and not gathered(sl, xs).any()
+        xs, it, nupd, res, status = g.cg_solve_mixed(c["param"], 0.0, 9, g.scatter(torch.from_numpy(b)), g.new_vectors())
+        assert it == 9 and status == 1
+        want = oracle.cg(c["dims"], 0, u, c["param"], 0.0, 9, b)
+        assert rel(gathered(sl, xs), want["x"]) <= 2e-5          # nine fp32 iterations against nine fp64 ones
+        # and the fp64 slab solver on the same slabs is not disturbed by the mixed one's state
+        xs, it, res, status = g.cg_solve(c["param"], c["tol"], 20000, g.scatter(torch.from_numpy(b)), g.new_vectors())
+        full = oracle.cg(c["dims"], 0, u, c["param"], c["tol"], 20000, b)
+        assert status == 0 and abs(it - full["iters"]) <= 2 and rel(gathered(sl, xs), full["x"]) <= CG_TOL
+    finally:
+        g.close()
+
+
+def test_slab_mixed_single_rank_entry_point(sl):
+    c, u, b = synth.config_inputs(1)
+    dims = c["dims"]
+    s = sl.Slab(dims, 0, 1)
+    try:
+        s.connect([s.mailbox_ptr])
+        ug = torch.from_numpy(u)
+        s.load_gauge(sl.local_gauge(ug, dims, 0, 1).cuda(), sl.u3_below_from_global(ug, dims, 0, 1).cuda())
+        want = oracle.cg(dims, 0, u, c["param"], c["tol"], 20000, b)
+        x, it, nupd, res, status = s.cg_solve_mixed(c["param"], c["tol"], 20000, torch.from_numpy(b).cuda(), s.new_vector())
+        assert status == 0 and res <= c["tol"] and nupd >= 1 and rel(x.cpu().numpy(), want["x"]) <= 1e-8
+    finally:
+        s.close()
+
+
 # ------------------------------------------------------------------ CUDA IPC plumbing, two processes on the one GPU
 def _ipc_worker(rank, world, port, out):
     """Maps the peer's mailbox through lqcd_slab_ipc_export / _open and moves bytes with plain copies.

@@ -58,6 +58,7 @@ def test_slab_memory_sizes(dims, nranks):
     v_local = dims[0] * dims[1] * dims[2] * (dims[3] // nranks)
     sh = slab.half_slice(dims)
     need = v_local * 576 + 18 * sh * 16 + 3 * (3 * v_local // 2) * 16     # links, ghost links, r p t
+    need += v_local * 288 + 18 * sh * 8 + 4 * (3 * v_local // 2) * 8      # fp32 copies of the mixed solver: links, ghost links, x r p t
     got = lib.lqcd_slab_workspace_bytes(s)
     assert need <= got <= need + 2 * 1024 * 1024 + v_local
     faces = 2 * 2 * 3 * sh * 16                                           # two buffers x two faces
