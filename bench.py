@@ -78,10 +78,11 @@ def ncu_traffic(key):
     ncu --set full capture (profiles/traffic.csv); None if that kernel/workload was not captured."""
     path = os.path.join(ROOT, "profiles", "traffic.csv")
     try:
-        for row in open(path).read().splitlines()[1:]:
-            f = row.split(",")
-            if f[0] == key:
-                return int(f[1]) + int(f[2])
+        rows = [row.split(",") for row in open(path).read().splitlines()[1:]]
+        for want in ("r02_" + key, key):   # the newest capture of that kernel / workload
+            for f in rows:
+                if f[0] == want:
+                    return int(f[1]) + int(f[2])
     except Exception:
         pass
     return None
@@ -555,6 +556,20 @@ def ours_line(args, cfg, metric, ranks, device, lqcd, torch, full=True):
     return line
 
 
+def all_configs_table(lines):
+    """Markdown table of an --all-configs run (one row per BASELINE.json config)."""
+    out = ["| config | CG time to solution | iterations | true residual | us per iteration | `value` GB/s | plain Dslash us "
+           "(GB/s, of measured copy peak) | e2e (host buffers) | SM clock MHz (reasons) |", "|---|---|---|---|---|---|---|---|---|"]
+    for l in lines:
+        e2e = "%.2f ms" % l["e2e"]["ms_per_step"] if l.get("e2e") else "--"
+        ck = l.get("clocks") or {}
+        out.append("| %s | %.3f ms | %d | %.2e | %.2f | %.0f | %.2f (%.0f, %.3f) | %s | %s (%s) |" % (
+            l["config"]["workload"], l["ms_per_step"], l["cg"]["iters"], l["cg"]["true_residual"], l["cg"]["us_per_iteration"],
+            l["value"], l["dslash"]["us_per_call"], l["dslash"]["GBps"], l["roofline"]["frac"], e2e,
+            ck.get("sm_mhz"), ",".join(ck.get("reasons") or []) or "none"))
+    return "\n".join(out) + "\n"
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -577,6 +592,7 @@ def main():
                          "(strong scaling; include/lqcd_slab.h; staggered configs)")
     ap.add_argument("--all-configs", action="store_true",
                     help="the five BASELINE.json configs in one run (no variants, no oracle timing): one JSON line with a list")
+    ap.add_argument("--table", default=None, help="with --all-configs: also write the five-config table (markdown) to this file")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -628,6 +644,9 @@ def main():
         lines = [ours_line(args, synth.config(n), metric, ranks, device, lqcd, torch, full=False) for n in (1, 2, 3, 4, 5)]
         if rank == 0:
             print(json.dumps({"metric": metric, "unit": "GB/s", "n_gpus": world, "all_configs": lines}))
+            if args.table:
+                with open(args.table, "w") as fh:
+                    fh.write(all_configs_table(lines))
         ranks.close()
         return 0
     line = ours_line(args, cfg, metric, ranks, device, lqcd, torch, full=True)
