@@ -520,6 +520,11 @@ def ours_line(args, cfg, metric, ranks, device, lqcd, torch, full=True):
         cpu = {"value": r["value"], "unit": "GB/s", "cores": r["cores"], "kind": "oracle", "sample": r["sample"],
                "dslash": oracle_dslash_times(cfg, u, b)}   # per call, all cores and one thread, beside dslash.us_per_call
 
+    if cpu is None and not full and rank == 0 and world == 1 and not args.no_cpu_baseline and cfg["name"] in ("cfg1", "cfg2", "cfg3"):
+        # --all-configs: the oracle's hopping term per call (all cores, one thread) for configs 1-3, SURVEY 8(d)
+        cpu = {"value": None, "unit": "GB/s", "kind": "oracle", "sample": "hopping term only",
+               "dslash": oracle_dslash_times(cfg, u, b, budget_s=2.0)}
+        cpu["cores"] = cpu["dslash"]["cores"]
     line = {
         "metric": metric, "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_solve, "higher_is_better": True, "scaling": "weak",
@@ -559,13 +564,16 @@ def ours_line(args, cfg, metric, ranks, device, lqcd, torch, full=True):
 def all_configs_table(lines):
     """Markdown table of an --all-configs run (one row per BASELINE.json config)."""
     out = ["| config | CG time to solution | iterations | true residual | us per iteration | `value` GB/s | plain Dslash us "
-           "(GB/s, of measured copy peak) | e2e (host buffers) | SM clock MHz (reasons) |", "|---|---|---|---|---|---|---|---|---|"]
+           "(GB/s, of measured copy peak) | oracle Dslash us per call: all cores / one thread | e2e (host buffers) | "
+           "SM clock MHz (reasons) |", "|---|---|---|---|---|---|---|---|---|---|"]
     for l in lines:
         e2e = "%.2f ms" % l["e2e"]["ms_per_step"] if l.get("e2e") else "--"
         ck = l.get("clocks") or {}
-        out.append("| %s | %.3f ms | %d | %.2e | %.2f | %.0f | %.2f (%.0f, %.3f) | %s | %s (%s) |" % (
+        od = (l.get("cpu_baseline") or {}).get("dslash")
+        ods = "%.0f (%d cores) / %.0f" % (od["us_per_call_all_cores"], od["cores"], od["us_per_call_one_thread"]) if od else "--"
+        out.append("| %s | %.3f ms | %d | %.2e | %.2f | %.0f | %.2f (%.0f, %.3f) | %s | %s | %s (%s) |" % (
             l["config"]["workload"], l["ms_per_step"], l["cg"]["iters"], l["cg"]["true_residual"], l["cg"]["us_per_iteration"],
-            l["value"], l["dslash"]["us_per_call"], l["dslash"]["GBps"], l["roofline"]["frac"], e2e,
+            l["value"], l["dslash"]["us_per_call"], l["dslash"]["GBps"], l["roofline"]["frac"], ods, e2e,
             ck.get("sm_mhz"), ",".join(ck.get("reasons") or []) or "none"))
     return "\n".join(out) + "\n"
 
