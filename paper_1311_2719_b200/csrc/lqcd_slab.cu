@@ -124,9 +124,9 @@ unsigned int vec_grid(const lqcd_slab* s)
 SlabVecPlan vec_plan(const lqcd_slab* s, unsigned int grid)
 {
     SlabVecPlan pl;
-    pl.n = s->nvec;
-    pl.nface = 6 * (size_t)s->sh < s->nvec ? 6 * (size_t)s->sh : s->nvec;
-    size_t fb = (pl.nface + kVecBlock - 1) / kVecBlock;
+    pl.n = (unsigned int)s->nvec;  // 3 Vh <= 3 * 2^29
+    pl.nface = 6 * (size_t)s->sh < s->nvec ? (unsigned int)(6 * (size_t)s->sh) : (unsigned int)s->nvec;
+    size_t fb = ((size_t)pl.nface + kVecBlock - 1) / kVecBlock;
     if (pl.nface == pl.n) fb = grid;               // no interior (T = 2): every block owns face elements
     else if (fb > grid / 2) fb = grid / 2;
     if (fb < 1) fb = 1;

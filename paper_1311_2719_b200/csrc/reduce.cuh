@@ -149,8 +149,8 @@ __device__ __forceinline__ void grid_sum(double local, const ReduceScratch& rs, 
 // finalisers that talk to other GPUs (slab_sync_tail).  `wrote_peer`: this thread stored into another
 // GPU's memory; a block in which any thread did fences at SYSTEM scope before it takes the ticket
 // (membar.sys in every block costs ~20 us on a 4096-block kernel, so only those blocks pay it).
-template <int BLOCK, class Finalise>
-__device__ __forceinline__ void grid_sum_block(double local, bool wrote_peer, const ReduceScratch& rs, Finalise fin)
+template <int BLOCK, class Early, class Finalise>
+__device__ __forceinline__ void grid_sum_block(double local, bool wrote_peer, const ReduceScratch& rs, Early early, Finalise fin)
 {
     __shared__ bool is_last_b;
     __shared__ double total_b;
@@ -168,6 +168,8 @@ __device__ __forceinline__ void grid_sum_block(double local, bool wrote_peer, co
     __syncthreads();
     if (is_last_b) {
         __threadfence();
+        // what the finaliser will need from memory is asked for now, so that it arrives while the partials are added
+        const auto e = early();
         double acc = 0.0;
         for (unsigned int i = threadIdx.x; i < gridDim.x; i += BLOCK) acc += __ldcg(rs.partials + i);
         double total = block_sum<BLOCK>(acc);
@@ -176,7 +178,7 @@ __device__ __forceinline__ void grid_sum_block(double local, bool wrote_peer, co
             total_b = total;
         }
         __syncthreads();
-        fin(total_b);
+        fin(total_b, e);
     }
 }
 

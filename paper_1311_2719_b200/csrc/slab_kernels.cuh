@@ -30,11 +30,11 @@ static __global__ void slab_signal_kernel(const SlabSyncArgs a)
     if ((int)threadIdx.x < a.nranks) slab_signal(a, a.ss->seq + 1, threadIdx.x);
 }
 
-static __global__ void slab_wait_combine_kernel(const SlabSyncArgs a) { slab_sync_point(a, false); }
+static __global__ void slab_wait_combine_kernel(const SlabSyncArgs a) { slab_sync_point(a, false, a.ss->seq); }
 
 // Both in one launch: what a rank that drives only its own slab enqueues (one process per GPU).
 // Never used by a group of several slabs on one stream, where every signal must precede every wait.
-static __global__ void slab_signal_wait_combine_kernel(const SlabSyncArgs a) { slab_sync_point(a, true); }
+static __global__ void slab_signal_wait_combine_kernel(const SlabSyncArgs a) { slab_sync_point(a, true, a.ss->seq); }
 
 
 // Where the two boundary time-slices of a slab vector go: element (c, e) of local slice 0 into the
@@ -56,53 +56,54 @@ typedef SlabPushT<cplxf> SlabPushF;  // fp32 vectors of the mixed-precision solv
 // fraction of the work of an interior block -- do so while the interior blocks are still streaming (round 1: the
 // fence sat on the kernel's tail, 28.6 us against 14.4 us for the same p-update without faces).
 struct SlabVecPlan {
-    size_t n, nface;   // elements, face elements (6 sh, or n if the slab has no interior)
-    int face_blocks;   // blocks [0, face_blocks) own the face elements, the others the interior
+    unsigned int n, nface;  // elements, face elements (6 sh, or n if the slab has no interior); n = 3 Vh < 2^31
+    int face_blocks;        // blocks [0, face_blocks) own the face elements, the others the interior
 };
 
-__device__ __forceinline__ void slab_vec_range(const SlabVecPlan& pl, size_t& v0, size_t& v1)
+// The walk of one block: v = v0 + threadIdx.x, v0 + threadIdx.x + step, ... < v1 -- a grid-stride walk inside the
+// block's group (faces or interior), so that at any moment the blocks of a group stream neighbouring addresses (one
+// contiguous run per block, as in round 1, cost 8 us of the 23 us p-update at 32^4 in DRAM locality).
+__device__ __forceinline__ void slab_vec_range(const SlabVecPlan& pl, int block, unsigned int& v0, unsigned int& v1, unsigned int& step)
 {
     if (gridDim.x == 1) {  // a single block walks everything, faces first
         v0 = 0;
         v1 = pl.n;
-        return;
-    }
-    if ((int)blockIdx.x < pl.face_blocks) {
-        const size_t per = (pl.nface + pl.face_blocks - 1) / pl.face_blocks;
-        v0 = (size_t)blockIdx.x * per;
-        v1 = v0 + per < pl.nface ? v0 + per : pl.nface;
-        if (v0 > pl.nface) v0 = pl.nface;
+        step = block;
+    } else if ((int)blockIdx.x < pl.face_blocks) {
+        v0 = blockIdx.x * block;
+        v1 = pl.nface;
+        step = pl.face_blocks * block;
     } else {
-        const size_t nint = pl.n - pl.nface, nb = gridDim.x - pl.face_blocks;
-        const size_t per = (nint + nb - 1) / nb;
-        v0 = pl.nface + (size_t)(blockIdx.x - pl.face_blocks) * per;
-        v1 = v0 + per < pl.n ? v0 + per : pl.n;
-        if (v0 > pl.n) v0 = pl.n;
+        v0 = pl.nface + (blockIdx.x - pl.face_blocks) * block;
+        v1 = pl.n;
+        step = (gridDim.x - pl.face_blocks) * block;
     }
 }
 
-// virtual index -> element index i = c Vh + e, and where (if anywhere) the element goes in the neighbours' ghosts
+// virtual index -> element index i = c Vh + e, and where (if anywhere) the element goes in the neighbours' ghosts.
+// 32-bit arithmetic throughout: with 64-bit divisions this index computation, not memory, bounded the kernel
+// (7 elements x 2 divisions per thread: 8 of the 23 us of the p-update at 32^4).
 template <class C>
-__device__ __forceinline__ size_t slab_vec_elem(const SlabPushT<C>& ph, const SlabVecPlan& pl, size_t v, C*& peer_dst)
+__device__ __forceinline__ unsigned int slab_vec_elem(const SlabPushT<C>& ph, const SlabVecPlan& pl, unsigned int v, C*& peer_dst)
 {
-    const size_t sh = (size_t)ph.sh, Vh = (size_t)ph.Vh;
+    const unsigned int sh = (unsigned int)ph.sh, Vh = (unsigned int)ph.Vh;
     peer_dst = nullptr;
     if (v < pl.nface) {
         if (Vh == 2 * sh) {  // T = 2: every site lies on a face, plain order; slice 0 -> lo, slice 1 -> hi
-            const size_t c = v / Vh, e = v - c * Vh;
-            peer_dst = e < sh ? ph.lo + c * sh + e : ph.hi + c * sh + (e - sh);
+            const unsigned int c = v / Vh, e = v - c * Vh;
+            peer_dst = e < sh ? ph.lo + (size_t)(c * sh + e) : ph.hi + (size_t)(c * sh + (e - sh));
             return v;
         }
-        const size_t f = v / sh, k = v - f * sh, c = f >> 1;
+        const unsigned int f = v / sh, k = v - f * sh, c = f >> 1;
         if (f & 1) {
-            peer_dst = ph.hi + c * sh + k;
+            peer_dst = ph.hi + (size_t)(c * sh + k);
             return c * Vh + (Vh - sh) + k;
         }
-        peer_dst = ph.lo + c * sh + k;
+        peer_dst = ph.lo + (size_t)(c * sh + k);
         return c * Vh + k;
     }
-    const size_t w = v - pl.nface, per = Vh - 2 * sh;
-    const size_t c = w / per;
+    const unsigned int w = v - pl.nface, per = Vh - 2 * sh;
+    const unsigned int c = w / per;
     return c * Vh + sh + (w - c * per);
 }
 
@@ -132,9 +133,9 @@ __global__ void __launch_bounds__(BLOCK) slab_cg_init_kernel(const cplx* __restr
 {
     double local = 0.0;
     bool wrote_peer = false;
-    size_t v0, v1;
-    slab_vec_range(pl, v0, v1);
-    for (size_t v = v0 + threadIdx.x; v < v1; v += BLOCK) {
+    unsigned int v0, v1, step;
+    slab_vec_range(pl, BLOCK, v0, v1, step);
+    for (unsigned int v = v0 + threadIdx.x; v < v1; v += step) {
         cplx* dst;
         const size_t i = slab_vec_elem(ph, pl, v, dst);
         const cplx val = b[i];
@@ -148,7 +149,8 @@ __global__ void __launch_bounds__(BLOCK) slab_cg_init_kernel(const cplx* __restr
         local += cnorm2(val);
     }
     if (fused)
-        grid_sum_block<BLOCK>(local, wrote_peer, rs, [&sy](double bb) { slab_sync_tail<BLOCK>(sy, bb); });
+        grid_sum_block<BLOCK>(local, wrote_peer, rs, [&sy]() { return sy.ss->seq; },
+                              [&sy](double bb, unsigned long long sq) { slab_sync_tail<BLOCK>(sy, bb, sq); });
     else
         grid_sum<BLOCK>(local, rs, [ss](double bb) { ss->part[0] = bb; });
 }
@@ -165,9 +167,9 @@ __global__ void __launch_bounds__(BLOCK) slab_cg_pupdate_kernel(const C* __restr
     const double beta = sc->beta;
     double local = 0.0;
     bool wrote_peer = false;
-    size_t v0, v1;
-    slab_vec_range(pl, v0, v1);
-    for (size_t v = v0 + threadIdx.x; v < v1; v += BLOCK) {
+    unsigned int v0, v1, step;
+    slab_vec_range(pl, BLOCK, v0, v1, step);
+    for (unsigned int v = v0 + threadIdx.x; v < v1; v += step) {
         C* dst;
         const size_t i = slab_vec_elem(ph, pl, v, dst);
         const double2 rv = to_d(r[i]);
@@ -183,7 +185,8 @@ __global__ void __launch_bounds__(BLOCK) slab_cg_pupdate_kernel(const C* __restr
         local += cnorm2(ps);
     }
     if (fused)
-        grid_sum_block<BLOCK>(local, wrote_peer, rs, [&sy](double pp) { slab_sync_tail<BLOCK>(sy, pp); });
+        grid_sum_block<BLOCK>(local, wrote_peer, rs, [&sy]() { return sy.ss->seq; },
+                              [&sy](double pp, unsigned long long sq) { slab_sync_tail<BLOCK>(sy, pp, sq); });
     else
         grid_sum<BLOCK>(local, rs, [ss](double pp) { ss->part[0] = pp; });
 }
@@ -197,9 +200,9 @@ __global__ void __launch_bounds__(BLOCK) slab_cg_init_mixed_kernel(const cplx* _
                                                                    SlabScalars* ss, ReduceScratch rs)
 {
     double local[2] = { 0.0, 0.0 };
-    size_t v0, v1;
-    slab_vec_range(pl, v0, v1);
-    for (size_t v = v0 + threadIdx.x; v < v1; v += BLOCK) {
+    unsigned int v0, v1, step;
+    slab_vec_range(pl, BLOCK, v0, v1, step);
+    for (unsigned int v = v0 + threadIdx.x; v < v1; v += step) {
         cplxf* dst;
         const size_t i = slab_vec_elem(ph, pl, v, dst);
         const cplx val = b[i];

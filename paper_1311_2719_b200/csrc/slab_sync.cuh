@@ -64,22 +64,25 @@ __device__ __forceinline__ void st_sys_u64(unsigned long long* p, unsigned long 
 {
     asm volatile("st.relaxed.sys.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
-__device__ __forceinline__ unsigned long long ld_acquire_sys_u64(const unsigned long long* p)
+// Polling load.  Relaxed is enough: the data IS the word (tag and payload in one single-copy-atomic 64-bit value), and
+// what the arrival of the words announces -- the ghost faces -- is read by a later kernel, never by this one.
+__device__ __forceinline__ unsigned long long ld_relaxed_sys_u64(const unsigned long long* p)
 {
     unsigned long long v;
-    asm volatile("ld.acquire.sys.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    asm volatile("ld.relaxed.sys.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
     return v;
 }
 
 // thread r < nranks: this rank's partial(s), tagged with the number of the synchronisation point, into rank r's
 // mailbox.  The faces were stored -- and fenced at system scope -- by the producer's blocks before this runs.
-__device__ __forceinline__ void slab_signal(const SlabSyncArgs& a, unsigned long long seq, int r)
+// own: the partial(s) in registers (fused tail), or null = read them from `part` (left there by the producer kernel).
+__device__ __forceinline__ void slab_signal(const SlabSyncArgs& a, unsigned long long seq, int r, const double* own = nullptr)
 {
     unsigned long long* dst = a.peer_word[r] + ((seq & 1ull) * a.nranks + a.rank) * 4;
     const unsigned long long tag = seq << 32;
     const int nv = a.nvals > 0 ? a.nvals : 1;  // a point without a sum still announces itself
     for (int k = 0; k < nv; ++k) {
-        const unsigned long long bits = a.nvals > 0 ? (unsigned long long)__double_as_longlong(a.ss->part[k]) : 0ull;
+        const unsigned long long bits = a.nvals > 0 ? (unsigned long long)__double_as_longlong(own ? own[k] : a.ss->part[k]) : 0ull;
         st_sys_u64(dst + 2 * k, tag | (bits & 0xffffffffull));
         st_sys_u64(dst + 2 * k + 1, tag | (bits >> 32));
     }
@@ -104,8 +107,8 @@ __device__ __forceinline__ bool slab_wait(const SlabSyncArgs& a, unsigned long l
     for (int k = 0; k < nv; ++k) {
         unsigned long long lo, hi;
         for (;;) {
-            lo = ld_acquire_sys_u64(src + 2 * k);
-            hi = ld_acquire_sys_u64(src + 2 * k + 1);
+            lo = ld_relaxed_sys_u64(src + 2 * k);
+            hi = ld_relaxed_sys_u64(src + 2 * k + 1);
             if ((lo >> 32) == tag && (hi >> 32) == tag) break;
             if (t0 == 0) t0 = slab_now_ns();
             if (slab_now_ns() - t0 > a.timeout_ns) return false;
@@ -200,15 +203,16 @@ __device__ __forceinline__ void slab_combine(const SlabSyncArgs& a, unsigned lon
 
 // signal + bounded wait + combine by the threads of one block (at least nranks of them): the body of every form
 // of a synchronisation point.  do_signal = false: the signal was sent by an earlier launch (group calls).
-__device__ __forceinline__ void slab_sync_point(const SlabSyncArgs& a, bool do_signal)
+// seq_done = the points this rank has completed (a.ss->seq, read by the caller); own: see slab_signal.
+__device__ __forceinline__ void slab_sync_point(const SlabSyncArgs& a, bool do_signal, unsigned long long seq_done, const double* own = nullptr)
 {
     __shared__ int sp_timed_out;
     __shared__ double sp_vals[kSlabMaxRanks][2];
-    const unsigned long long seq = a.ss->seq + 1;
+    const unsigned long long seq = seq_done + 1;
     if (threadIdx.x == 0) sp_timed_out = 0;
     __syncthreads();
     if ((int)threadIdx.x < a.nranks) {
-        if (do_signal) slab_signal(a, seq, threadIdx.x);
+        if (do_signal) slab_signal(a, seq, threadIdx.x, own);
         double v[2];
         if (!slab_wait(a, seq, threadIdx.x, v)) sp_timed_out = 1;
         sp_vals[threadIdx.x][0] = v[0];
@@ -218,17 +222,16 @@ __device__ __forceinline__ void slab_sync_point(const SlabSyncArgs& a, bool do_s
     if (threadIdx.x == 0) slab_combine(a, seq, sp_timed_out != 0, sp_vals);
 }
 
-// The whole synchronisation point run by the LAST block of a producer kernel (`total` = this rank's
-// partial sum, known to every thread of that block): what a rank that drives only its own slab uses
-// instead of separate launches -- the halo exchange, the all-reduce and the scalar step of the CG
-// then cost no kernel boundary at all.  Every block of the producer has fenced its face stores at
-// system scope before taking the reduction ticket, so they are visible to a peer that sees the flag.
+// The whole synchronisation point run by the LAST block of a producer kernel (`total` = this rank's partial sum,
+// known to every thread of that block; seq_done was read while the partials were being added): what a rank that
+// drives only its own slab uses instead of separate launches -- the halo exchange, the all-reduce and the scalar step
+// of the CG then cost no kernel boundary at all.  Every block of the producer that stored faces has fenced them at
+// system scope before taking the reduction ticket, so they are visible to a peer that sees the words.
 template <int BLOCK>
-__device__ __forceinline__ void slab_sync_tail(const SlabSyncArgs& a, double total)
+__device__ __forceinline__ void slab_sync_tail(const SlabSyncArgs& a, double total, unsigned long long seq_done)
 {
-    if (threadIdx.x == 0) a.ss->part[0] = total;
-    __syncthreads();
-    slab_sync_point(a, true);
+    const double own[2] = { total, 0.0 };
+    slab_sync_point(a, true, seq_done, own);
 }
 
 }  // namespace lqcd

@@ -261,7 +261,8 @@ __device__ __forceinline__ void stag_dslash_body(const StagArgs<C>& a, const Sla
             }
         }
         if (sy != nullptr) {
-            grid_sum_block<BLOCK>(local, wrote_peer, a.rs, [sy](double v) { slab_sync_tail<BLOCK>(*sy, v); });
+            grid_sum_block<BLOCK>(local, wrote_peer, a.rs, [sy]() { return sy->ss->seq; },
+                                  [sy](double v, unsigned long long sq) { slab_sync_tail<BLOCK>(*sy, v, sq); });
         } else {
             double* part = a.sl.part;
             grid_sum<BLOCK>(local, a.rs, [part](double v) { part[0] = v; });
