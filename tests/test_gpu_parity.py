@@ -213,6 +213,34 @@ def test_cg_persistent_kernel_changes_no_bit(lq, dims, recon, every):
     assert abs(p[1] - want["iters"]) <= 2 and rel(p[0], want["x"]) <= CG_TOL
 
 
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (6, 4, 2, 2), (8, 8, 8, 4)])
+def test_wilson_cg_modes_and_the_x_update_in_the_vector_kernel(lq, dims):
+    """The Wilson CG does x += alpha p in the vector kernel that follows the update of r (cg_xpupdate_kernel).  The
+    three host loops must give the same bits -- the synchronous one launches that kernel once more after the exit
+    rule has fired -- and an exit by maxiter must not lose the last update: x_k against the oracle's x_k."""
+    kappa = 0.12
+    u = synth.gauge_field(dims, "smooth", 41)
+    b = synth.source(dims, "wilson", 42)
+    want = oracle.cg(dims, 1, u, kappa, 1e-10, 20000, b)
+    with make_lattice(lq, dims, 1, u) as lat:
+        got = []
+        for mode, every in ((lq.CG_SYNC, 1), (lq.CG_ASYNC, 1), (lq.CG_ASYNC, 5), (lq.CG_GRAPH, 8)):
+            lat.set_option(lq.OPT_CG_MODE, mode)
+            lat.set_option(lq.OPT_CG_CHECK_EVERY, every)
+            x, it, res, status = lat.cg_solve(kappa, 1e-10, 20000, dev(b))
+            got.append((host(x), it, res, status, lat.cg_history().numpy()))
+            for k in (1, 6):
+                xk, itk, _, stk = lat.cg_solve(kappa, 0.0, k, dev(b))
+                wk = oracle.cg(dims, 1, u, kappa, 0.0, k, b)
+                assert itk == k and stk == 1 and rel(host(xk), wk["x"]) <= 1e-12
+            xz, itz, resz, stz = lat.cg_solve(kappa, 1e-10, 100, dev(np.zeros_like(b)))
+            assert itz == 0 and resz == 0.0 and stz == 0 and not host(xz).any()
+    x, it, res, status, h = got[0]
+    assert status == 0 and abs(it - want["iters"]) <= 2 and rel(x, want["x"]) <= CG_TOL
+    for o in got[1:]:
+        assert np.array_equal(o[0], x) and o[1:4] == (it, res, status) and np.array_equal(o[4], h)
+
+
 @pytest.mark.parametrize("mode", [0, 1, 2])
 def test_cg_fixed_iteration_count_matches_oracle_iterate(lq, mode):
     """tol = 0 runs exactly maxiter iterations: compare the iterate x_k itself."""
