@@ -226,46 +226,81 @@ def slab_group_variant(slab_mod, cfg, ug, bg, R, args, maxiter, mixed=False):
 
 def slab_strong_variant(args, cfg, ranks, device, maxiter):
     """One solve of cfg as N time-slabs, one per rank/GPU (collective: every rank calls it).  Returns a dict on every
-    rank; an {"error": ...} dict if anything fails on any rank."""
+    rank; an {"error": ...} dict on EVERY rank if anything fails on any rank.  Failure-safe by construction: after each
+    phase that can fail locally the ranks agree (an all-reduce every rank reaches) whether to go on, the waits inside
+    the solver are bounded (LQCD_ECOMM), so no rank is ever left in a collective its peers have abandoned."""
     import torch
     from paper_1311_2719_b200 import slab as sl
     rank, world = ranks.rank, ranks.world
     dims = cfg["dims"]
-    out, s = None, None
-    try:
-        if dims[3] % world or (dims[3] // world) % 2 or dims[3] // world < 2:
-            raise ValueError("L3 = %d cannot be cut into %d even slabs" % (dims[3], world))
+    if dims[3] % world or (dims[3] // world) % 2 or dims[3] // world < 2:   # the same verdict on every rank
+        return {"error": "L3 = %d cannot be cut into %d even slabs" % (dims[3], world)}
+    state = {"s": None, "why": ""}
+
+    def agreed(step):
+        """Run a local step; then every rank learns whether all of them succeeded."""
+        bad = 0.0
+        try:
+            step()
+        except Exception as exc:  # noqa: BLE001
+            state["why"] = repr(exc)[:300]
+            bad = 1.0
+        return ranks.sum(bad) == 0
+
+    def give_up(where):
+        try:
+            if state["s"] is not None:
+                state["s"].close()
+        except Exception:  # noqa: BLE001
+            pass
+        return {"error": "%s: %s" % (where, state["why"] or "a peer failed")}
+
+    def create():
         ug = torch.from_numpy(synth.gauge_field(dims, cfg["links"], cfg["seed"]))
         bg = torch.from_numpy(synth.source(dims, cfg["fermion"], cfg["seed"]))
         s = sl.Slab(dims, rank, world, device=device)
+        state["s"] = s
         s.set_option(sl.OPT_RECONSTRUCT, args.recon)
         s.set_option(sl.OPT_CHECK_EVERY, args.check_every)
         s.set_option(sl.OPT_TIMEOUT_MS, 10000)
-        s.connect_ipc()
-        s.load_gauge(sl.local_gauge(ug, dims, rank, world).to(device), sl.u3_below_from_global(ug, dims, rank, world).to(device))
-        b_dev, x_dev = sl.local_vector(bg, dims, rank, world).to(device), s.new_vector()
-        del ug, bg
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        for rep in range(2):   # one warm-up, one timed
-            ranks.barrier()
+        state["u"] = (sl.local_gauge(ug, dims, rank, world), sl.u3_below_from_global(ug, dims, rank, world))
+        state["b"] = sl.local_vector(bg, dims, rank, world)
+
+    if not agreed(create):
+        return give_up("set-up")
+    if not agreed(lambda: state["s"].connect_ipc()):   # itself collective and failure-safe (slab.py)
+        return give_up("connect_ipc")
+    s = state["s"]
+
+    def load():
+        s.load_gauge(state["u"][0].to(device), state["u"][1].to(device))
+        state["bd"], state["xd"] = state["b"].to(device), s.new_vector()
+
+    if not agreed(load):
+        return give_up("load_gauge")
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for rep in range(2):   # one warm-up, one timed
+
+        def solve():
             e0.record(s.stream)
-            _, it, res, st = s.cg_solve(cfg["param"], cfg["tol"], maxiter, b_dev, x_dev)
+            state["res"] = s.cg_solve(cfg["param"], cfg["tol"], maxiter, state["bd"], state["xd"])
             e1.record(s.stream)
-            ranks.barrier()
-        ms = ranks.max(e0.elapsed_time(e1))
-        sh = dims[0] * dims[1] * dims[2] // 2
-        out = {"time_to_solution_ms": ms, "iters": it, "true_residual": res, "converged": st == 0,
-               "GBps": cg_bytes(cfg, it, args.recon) / (ms * 1e-3) / 1e9, "scaling": "strong",
-               "nvlink_bytes_per_dslash_and_rank": 2 * sh * 48, "sync_points": s.sync_points(),
-               "note": "one system, T = %d time-slices per GPU; first multi-GPU run of this path: check against the N = 1 solve" % (dims[3] // world)}
-    except Exception as exc:  # noqa: BLE001
-        out = {"error": repr(exc)[:300]}
-    finally:
-        try:
-            if s is not None:
-                s.close()
-        except Exception:  # noqa: BLE001
-            pass
+            torch.cuda.synchronize(device)
+
+        ranks.barrier()
+        if not agreed(solve):
+            return give_up("cg_solve")
+    _, it, res, st = state["res"]
+    ms = ranks.max(e0.elapsed_time(e1))
+    sh = dims[0] * dims[1] * dims[2] // 2
+    out = {"time_to_solution_ms": ms, "iters": it, "true_residual": res, "converged": st == 0,
+           "GBps": cg_bytes(cfg, it, args.recon) / (ms * 1e-3) / 1e9, "scaling": "strong",
+           "nvlink_bytes_per_dslash_and_rank": 2 * sh * 48, "sync_points": s.sync_points(),
+           "note": "one system, T = %d time-slices per GPU; first multi-GPU run of this path: check against the N = 1 solve" % (dims[3] // world)}
+    try:
+        s.close()
+    except Exception:  # noqa: BLE001
+        pass
     return out
 
 

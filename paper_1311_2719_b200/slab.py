@@ -205,33 +205,49 @@ class Slab:
 
     def connect_ipc(self, group=None):
         """One process per GPU on one node: all-gather the CUDA IPC handles of the mailboxes and map the
-        peers' (torch.distributed is the transport of the 72 bytes per rank; set-up time only)."""
+        peers' (torch.distributed is the transport of the 73 bytes per rank; set-up time only).
+        Collective and failure-safe: a rank whose export or open fails still takes part in every collective
+        of this call, and then EVERY rank raises -- no rank is left waiting for one that has given up."""
         import torch.distributed as dist
         if self.nranks == 1:
             self.connect([self.mailbox_ptr])
             return
+        dev = self.device if dist.get_backend(group) == "nccl" else torch.device("cpu")
+        failure = ""
         handle = ctypes.create_string_buffer(64)
         off = ctypes.c_size_t()
-        self._check(self._lib.lqcd_slab_ipc_export(self._s, handle, ctypes.byref(off)))
-        mine = torch.tensor(list(handle.raw) + list(int(off.value).to_bytes(8, "little")), dtype=torch.uint8)
-        dev = self.device if dist.get_backend(group) == "nccl" else torch.device("cpu")
-        mine = mine.to(dev)
+        try:
+            self._check(self._lib.lqcd_slab_ipc_export(self._s, handle, ctypes.byref(off)))
+        except Exception as exc:  # noqa: BLE001 - reported to every rank below
+            failure = "export: %r" % (exc,)
+        mine = torch.tensor(list(handle.raw) + list(int(off.value).to_bytes(8, "little")) + [0 if not failure else 1],
+                            dtype=torch.uint8).to(dev)
         everyone = [torch.empty_like(mine) for _ in range(self.nranks)]
         dist.all_gather(everyone, mine, group=group)
+        raws = [bytes(t.cpu().tolist()) for t in everyone]
+        if not failure and any(r[72] for r in raws):
+            failure = "a peer could not export its mailbox"
         ptrs = []
-        for r, t in enumerate(everyone):
-            if r == self.rank:
-                ptrs.append(self.mailbox_ptr)
-                continue
-            raw = bytes(t.cpu().tolist())
-            out = ctypes.c_void_p()
-            o = int.from_bytes(raw[64:72], "little")
-            self._check(self._lib.lqcd_slab_ipc_open(self._s, raw[:64], o, ctypes.byref(out)))
-            self._opened.append((out.value, o))
-            ptrs.append(out.value)
-        self.connect(ptrs)
-        torch.cuda.synchronize(self.device)
-        dist.barrier(group=group)  # every mailbox is zeroed and mapped before anyone's first compute call
+        if not failure:
+            try:
+                for r, raw in enumerate(raws):
+                    if r == self.rank:
+                        ptrs.append(self.mailbox_ptr)
+                        continue
+                    out = ctypes.c_void_p()
+                    o = int.from_bytes(raw[64:72], "little")
+                    self._check(self._lib.lqcd_slab_ipc_open(self._s, raw[:64], o, ctypes.byref(out)))
+                    self._opened.append((out.value, o))
+                    ptrs.append(out.value)
+                self.connect(ptrs)
+                torch.cuda.synchronize(self.device)
+            except Exception as exc:  # noqa: BLE001
+                failure = "open: %r" % (exc,)
+        # every mailbox is zeroed and mapped before anyone's first compute call -- or nobody goes on
+        ok = torch.tensor([0 if failure else 1], dtype=torch.int32).to(dev)
+        dist.all_reduce(ok, op=dist.ReduceOp.MIN, group=group)
+        if int(ok.item()) == 0:
+            raise LqcdError(ECOMM, "rank %d: mailboxes not connected (%s)" % (self.rank, failure or "a peer failed"))
 
     def new_vector(self) -> torch.Tensor:
         return torch.zeros(self.vector_shape, dtype=torch.complex128, device=self.device)
