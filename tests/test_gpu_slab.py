@@ -403,6 +403,29 @@ def test_slab_mixed_cg_agrees_with_the_single_gpu_mixed_solver_and_batching(sl):
         g.close()
 
 
+@pytest.mark.slow
+@pytest.mark.parametrize("recon", [18, 12])
+def test_slab_mixed_cg_cfg3_bench_workload(sl, recon, cfg3_inputs, cfg3_oracle_cg):
+    """The bench workload (32^4, m = 0.01) through the mixed-precision slab solver in two slabs, against the oracle's
+    fp64 CG on the undivided lattice (run once per session): the contract of DESIGN.md 9.3 -- true residual <= tol,
+    the WHOLE solution within 1e-8 -- plus the stored 4096-entry sample and one oracle application of A."""
+    c, u, b = cfg3_inputs
+    dims = c["dims"]
+    g = group_for(sl, dims, 2, u, recon)
+    try:
+        xs, it, nupd, res, status = g.cg_solve_mixed(c["param"], c["tol"], 50000, g.scatter(torch.from_numpy(b)), g.new_vectors())
+        x = gathered(sl, xs)
+    finally:
+        g.close()
+    want = cfg3_oracle_cg
+    assert status == 0 and res <= c["tol"] and nupd >= 5
+    assert _count_close(it, want["iters"])             # reliable updates cost no convergence (3141 against 3138 undivided)
+    assert rel(x, want["x"]) <= 1e-8
+    check_sampled_solution(x, golden("cfg3"), 1e-8)
+    ax = oracle.apply_MdagM(dims, 0, u, c["param"], x)
+    assert abs(rel(ax, b) - res) <= 1e-3 * res + 1e-13
+
+
 def test_slab_mixed_single_rank_entry_point(sl):
     c, u, b = synth.config_inputs(1)
     dims = c["dims"]
