@@ -548,6 +548,28 @@ def ours_line(args, cfg, metric, ranks, device, lqcd, torch, full=True):
             except Exception as exc:  # noqa: BLE001
                 variants["slab_group2_mixed_on_one_gpu"] = {"error": repr(exc)[:200]}
 
+    if f == lqcd.WILSON and not args.no_variants and full:
+        # the even-odd (Schur) preconditioned solver of the same system M x = b, and two-row links
+        variants = {}
+        for recon_v in (args.recon, 30 - args.recon):
+            lat.set_option(lqcd.OPT_RECONSTRUCT, recon_v)
+            lat.load_gauge(u_dev)
+            for name_v, call_v in (("eo_solve", lambda: lat.wilson_solve_eo(cfg["param"], cfg["tol"], maxiter, b_dev)),
+                                   ("f64", lambda: lat.cg_solve(cfg["param"], cfg["tol"], maxiter, b_dev, x_dev))):
+                if name_v == "f64" and recon_v == args.recon:
+                    continue   # the headline itself
+                call_v()
+                v0, v1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                barrier()
+                v0.record(lat.stream)
+                _, it_v, res_v, st_v = call_v()
+                v1.record(lat.stream)
+                barrier()
+                variants["%s_recon%d" % (name_v, recon_v)] = {"time_to_solution_ms": max_over_ranks(v0.elapsed_time(v1)), "iters": it_v,
+                                                              "true_residual": res_v, "converged": st_v == 0}
+        lat.set_option(lqcd.OPT_RECONSTRUCT, args.recon)
+        lat.load_gauge(u_dev)
+
     # ---- the oracle beside it (rank 0, N = 1 only)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline and full:
