@@ -54,6 +54,8 @@ def lib():
         L.oracle_apply_MdagM.argtypes = [P, ctypes.c_int, P, ctypes.c_double, P, P]
         L.oracle_dot_re.argtypes = [P, P, ctypes.c_long]
         L.oracle_dot_re.restype = ctypes.c_double
+        L.oracle_dot_re_f.argtypes = [P, P, ctypes.c_long]
+        L.oracle_dot_re_f.restype = ctypes.c_double
         L.oracle_cg.argtypes = [P, ctypes.c_int, P, ctypes.c_double, ctypes.c_double, ctypes.c_int, P, P, P, P, P]
         L.oracle_stag_M.argtypes = [P, P, ctypes.c_double, P, P, P, P]
         L.oracle_stag_solve_full.argtypes = [P, P, ctypes.c_double, ctypes.c_double, ctypes.c_int, P, P, P, P, P, P]
@@ -166,6 +168,13 @@ def dot_re(a, b) -> float:
     a = _c(a, np.complex128)
     b = _c(b, np.complex128)
     return lib().oracle_dot_re(_ptr(a), _ptr(b), a.size)
+
+
+def dot_re_f(a, b) -> float:
+    """Re<fl32(a), fl32(b)> accumulated in fp64: the inner product of the mixed-precision CG."""
+    a = _c(a, np.complex128)
+    b = _c(b, np.complex128)
+    return lib().oracle_dot_re_f(_ptr(a), _ptr(b), a.size)
 
 
 def cg(dims, fermion, u, param, tol, maxiter, b, history=False):

@@ -699,6 +699,29 @@ static double dot_re_f(const cf *a, const cf *b, long n)
     return s;
 }
 
+/* dot_re_f through the C interface, for its own pin (tests/test_oracle_mixed.py): the fp64 arguments are
+ * rounded to fp32 and handed to dot_re_f as the mixed-precision CG hands it rs, ps, ts.  No arithmetic of
+ * its own.  Returns NaN if the two temporaries cannot be allocated. */
+double oracle_dot_re_f(const double *a_, const double *b_, long n_complex)
+{
+    const cd *a = (const cd *)a_, *b = (const cd *)b_;
+    const long n = n_complex > 0 ? n_complex : 0;
+    cf *af = malloc(sizeof(cf) * (n > 0 ? n : 1)), *bf = malloc(sizeof(cf) * (n > 0 ? n : 1));
+    if (!af || !bf) {
+        free(af);
+        free(bf);
+        return NAN;
+    }
+    for (long i = 0; i < n; ++i) {
+        af[i] = (cf)a[i];
+        bf[i] = (cf)b[i];
+    }
+    const double s = dot_re_f(af, bf, n);
+    free(af);
+    free(bf);
+    return s;
+}
+
 /* The fp32 hopping term through the C interface (for its own pin against the fp64 one). */
 int oracle_stag_dslash_f32(const int *L, const double *u_, int out_parity, const double *in_, double *out_)
 {

@@ -87,3 +87,45 @@ def test_mixed_cg_edge_cases():
     assert r0["status"] == 1 and r0["iters"] == 40 and r0["updates"] >= 1
     with pytest.raises(ValueError):
         oracle.cg_mixed(dims, u, 0.1, 1e-10, 10, b, delta=1.5)
+
+
+@pytest.mark.parametrize("n", [1, 17, 4096, 4097, 3 * 4096 + 17])
+def test_fp32_inner_product_over_several_blocks_and_a_ragged_tail(n):
+    """oracle.dot_re_f supplies every alpha, beta and update decision of oracle.cg_mixed (the
+    sums) and adds in fixed 4096-element blocks like dot_re; the 16^4 and larger mixed runs (and the stored
+    cfgN_mixed counts) go through the block loop.  Pinned against numpy's own product of the SAME fp32-rounded
+    numbers -- exactly representable in fp64, so only the order of the additions differs -- at one element,
+    under one block, one block exactly, one block + 1, and several blocks + a ragged tail."""
+    rng = np.random.default_rng(2200 + n)
+    a = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    b = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    a32 = a.astype(np.complex64).astype(np.complex128)
+    b32 = b.astype(np.complex64).astype(np.complex128)
+    scale = np.linalg.norm(a32) * np.linalg.norm(b32)
+    want = np.vdot(a32, b32).real
+    assert abs(oracle.dot_re_f(a, b) - want) <= 1e-14 * scale
+    assert abs(oracle.dot_re_f(a, a) - np.linalg.norm(a32) ** 2) <= 1e-14 * scale
+    # it really rounds to fp32 first: the fp64 product of the unrounded numbers is ~1e-8 away, not 1e-16
+    if n >= 17:
+        assert abs(oracle.dot_re_f(a, a) - np.linalg.norm(a) ** 2) > 1e-10 * np.linalg.norm(a) ** 2
+    # every block counts, the last one included: a vector that is zero except in its last element
+    e = np.zeros(n, complex)
+    e[-1] = 3.0 - 4.0j
+    assert oracle.dot_re_f(e, e) == 25.0
+    assert oracle.dot_re_f(e, 1j * e) == 0.0
+
+
+def test_mixed_cg_on_a_system_longer_than_one_block():
+    """BASELINE.json config 2 (16^4: 98 304 complex per vector = 24 blocks of the inner products): the mixed
+    oracle against the plain fp64 oracle CG (pinned by P7 and the residual tests) within the DESIGN.md 9.3
+    bound, and its reported residual against one retaken here in numpy from the fp64 operator."""
+    c, u, b = synth.config_inputs(2)
+    dims, mass, tol = c["dims"], c["param"], c["tol"]
+    want = oracle.cg(dims, STAGGERED, u, mass, tol, 20000, b)
+    r = oracle.cg_mixed(dims, u, mass, tol, 20000, b)
+    assert r["status"] == 0 and r["updates"] >= 2
+    res = np.linalg.norm(b - oracle.apply_MdagM(dims, STAGGERED, u, mass, r["x"])) / np.linalg.norm(b)
+    assert res <= tol and abs(res - r["true_residual"]) <= 1e-6 * res
+    bound = 2 * tol * np.linalg.norm(b) / mass ** 2 / np.linalg.norm(want["x"])
+    assert rel(r["x"], want["x"]) <= min(bound, 1e-8)
+    assert want["iters"] <= r["iters"] + 2 and r["iters"] <= 1.25 * want["iters"] + 10
