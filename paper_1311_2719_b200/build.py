@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "liblqcd_b200.so")
-SOURCES = [os.path.join(CSRC, "lqcd_api.cu"), os.path.join(CSRC, "lqcd_slab.cu")]
+SOURCES = [os.path.join(CSRC, "lqcd_api.cu"), os.path.join(CSRC, "lqcd_slab.cu"), os.path.join(CSRC, "lqcd_noalloc.cu")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-lineinfo", "-std=c++17",
@@ -19,7 +19,8 @@ NVCC_FLAGS = [
 
 
 def _deps():
-    out = [os.path.join(ROOT, "include", "lqcd.h"), os.path.join(ROOT, "include", "lqcd_slab.h"), os.path.abspath(__file__)]
+    out = [os.path.join(ROOT, "include", "lqcd.h"), os.path.join(ROOT, "include", "lqcd_slab.h"),
+           os.path.join(ROOT, "include", "lqcd_noalloc.h"), os.path.abspath(__file__)]
     for f in os.listdir(CSRC):
         if f.endswith((".cu", ".cuh", ".h")):
             out.append(os.path.join(CSRC, f))
