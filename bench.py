@@ -40,6 +40,21 @@ WILSON_DSLASH_BYTES = 1536
 WILSON_DSLASH_FLOPS = 1320
 NOMINAL_HBM_GBS = 8000.0
 FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
+L2_BYTES = 126e6           # B200 L2 (B200_PROFILING.md); the library's own rule reads cudaDevAttrL2CacheSize
+
+
+def links_fit_l2(cfg, recon: int) -> bool:
+    """The library's rule for the one-kernel loop (lqcd_load_gauge): the stored links take at most a third of the L2."""
+    return synth.volume(cfg["dims"]) * 4 * (recon // 2) * 16 <= L2_BYTES / 3
+
+
+def expected_cg_path(args, cfg) -> str:
+    """Which iteration loop lqcd_cg_solve runs for these flags (LQCD_OPT_PERSISTENT = -1, automatic): the one
+    cooperative kernel where the links fit the L2 -- staggered fp64 solves only, and never against an explicit
+    --cg-mode sync -- else the host loop in the --cg-mode form.  ours_line checks it against lqcd_last_cg_path()."""
+    if cfg["fermion"] == "staggered" and args.precision == "f64" and args.cg_mode != "sync" and links_fit_l2(cfg, args.recon):
+        return "persistent"
+    return "host_loop"
 
 
 def cg_bytes(cfg, iters: int, recon: int = 18, updates: int = -1) -> float:
@@ -139,11 +154,24 @@ def workload_name(cfg):
 def config_dict(args, cfg, world):
     """The `config` object of the JSON line: the same keys and values in our arm and in the reference arm
     (what the reference arm samples of the workload is said in its cpu_baseline.sample)."""
-    v = synth.volume(cfg["dims"])
+    link_mb = synth.volume(cfg["dims"]) * 4 * (args.recon // 2) * 16 / 1e6
+    path = expected_cg_path(args, cfg)
+    if path == "persistent":
+        mode = "persistent: the loop is one cooperative kernel, exit test on the device (cg_mode %s / check_every %d not used)" % (
+            args.cg_mode, args.check_every)
+    else:
+        mode = args.cg_mode
+    if link_mb * 1e6 > L2_BYTES:
+        l2 = "inputs larger than L2 (%.0f MB of links per Dslash against %.0f MB), no flush" % (link_mb, L2_BYTES / 1e6)
+    elif path == "persistent":
+        l2 = "L2-RESIDENT workload by design (%.1f MB of links fit the %.0f MB L2; no flush): the times are L2 times, not HBM times" % (
+            link_mb, L2_BYTES / 1e6)
+    else:
+        l2 = "%.0f MB of links against %.0f MB of L2: partly L2-resident, no flush" % (link_mb, L2_BYTES / 1e6)
     return {"workload": workload_name(cfg), "precision": args.precision, "reconstruct": args.recon,
-            "cg_mode": args.cg_mode, "check_every": args.check_every,
+            "cg_mode": mode, "cg_path": path, "check_every": args.check_every if path == "host_loop" else None,
             "parallelism": "replicas x%d (independent right-hand sides)" % world,
-            "l2_policy": "inputs larger than L2 (%.0f MB of links per Dslash), no flush" % (v * 576 / 1e6)}
+            "l2_policy": l2}
 
 
 def oracle_dslash_times(cfg, u, b, budget_s=4.0):
@@ -401,9 +429,12 @@ def slab_arm(args, cfg, workload, metric, ranks, device):
     return 0
 
 
-def ours_line(args, cfg, metric, ranks, device, lqcd, torch, full=True):
-    """Our arm on one config: returns the JSON line (a dict) on every rank.  full = False (--all-configs):
-    no solver variants, no oracle timing."""
+def ours_line(args, cfg, metric, ranks, device, lqcd, torch, full=True, solver_variants=None):
+    """Our arm on one config: returns the JSON line (a dict) on every rank.  full = False (--all-configs, and the
+    `configs` entries of the default line): no oracle timing, no slab variants, and the other solvers on the same
+    workload (two-row links, mixed precision; Wilson: the even-odd solve) only if solver_variants is set."""
+    if solver_variants is None:
+        solver_variants = full
     rank, world, local_rank = ranks.rank, ranks.world, ranks.local_rank
     barrier, max_over_ranks, sum_over_ranks = ranks.barrier, ranks.max, ranks.sum
     workload = workload_name(cfg)
@@ -442,6 +473,7 @@ def ours_line(args, cfg, metric, ranks, device, lqcd, torch, full=True):
     for _ in range(max(args.warmup, 3)):
         iters, updates, res, status = solve()
     assert status == 0, "CG did not converge"
+    path_ran = {lqcd.PATH_HOST_LOOP: "host_loop", lqcd.PATH_PERSISTENT: "persistent"}.get(lat.last_cg_path(), "none")
 
     # ---- timed region 1: K whole solves, device-resident inputs
     sampler = ClockSampler(local_rank) if rank == 0 else None
@@ -503,7 +535,7 @@ def ours_line(args, cfg, metric, ranks, device, lqcd, torch, full=True):
 
     # ---- the other solver variants on the same workload: time-to-solution only (one warm-up, one timed solve)
     variants = None
-    if f == lqcd.STAGGERED and not args.no_variants and full:
+    if f == lqcd.STAGGERED and not args.no_variants and solver_variants:
         variants = {}
         for recon_v, prec_v in ((18, "f64"), (12, "f64"), (18, "mixed"), (12, "mixed")):
             if (recon_v, prec_v) == (args.recon, args.precision):
@@ -533,7 +565,7 @@ def ours_line(args, cfg, metric, ranks, device, lqcd, torch, full=True):
         # lock-step on one stream: the kernels, peer stores and mailboxes of an R-GPU run, so the
         # difference to the undivided solve is the cost of the decomposition itself (6 tiny kernels
         # per iteration, smaller grids), not of any link.  One warm-up + one timed solve each.
-        if world == 1 and not mixed:
+        if world == 1 and not mixed and full:
             from paper_1311_2719_b200 import slab as slab_mod
             ug, bg = torch.from_numpy(u), torch.from_numpy(b)
             for R in (2, 4, 8):
@@ -548,7 +580,7 @@ def ours_line(args, cfg, metric, ranks, device, lqcd, torch, full=True):
             except Exception as exc:  # noqa: BLE001
                 variants["slab_group2_mixed_on_one_gpu"] = {"error": repr(exc)[:200]}
 
-    if f == lqcd.WILSON and not args.no_variants and full:
+    if f == lqcd.WILSON and not args.no_variants and solver_variants:
         # the even-odd (Schur) preconditioned solver of the same system M x = b, and two-row links
         variants = {}
         for recon_v in (args.recon, 30 - args.recon):
@@ -589,7 +621,7 @@ def ours_line(args, cfg, metric, ranks, device, lqcd, torch, full=True):
         "data": "synthetic",
         "config": config_dict(args, cfg, world),
         "cg": {"time_to_solution_ms": ms_solve, "iters": iters, "reliable_updates": updates if mixed else None,
-               "true_residual": res,
+               "true_residual": res, "path": path_ran,   # lqcd_last_cg_path(): the loop that really ran
                "us_per_iteration": ms_solve * 1e3 / max(iters, 1)},
         "dslash": {"us_per_call": us_dslash, "GBps": achieved, "GFLOPs": dflops * sites_out / (us_dslash * 1e-6) / 1e9,
                    "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS, "reps": args.dslash_reps},
@@ -603,6 +635,9 @@ def ours_line(args, cfg, metric, ranks, device, lqcd, torch, full=True):
                      "bytes_per_site": dbytes, "sites_per_launch": sites_out},
         "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "cpu_baseline": cpu, "variants": variants,
     }
+    if path_ran != line["config"]["cg_path"]:   # the library chose otherwise than bench.py's copy of its rule: say so
+        line["config"]["cg_path"] = path_ran
+        line["config"]["cg_mode"] = "%s (lqcd_last_cg_path: %s)" % (args.cg_mode, path_ran)
     line["roofline"]["traffic"] = ncu_traffic("%s_dslash_plain%s" % (cfg["name"], "" if args.recon == 18 else "_recon12"))
     if line["roofline"]["traffic"] is not None:
         line["roofline"]["traffic_source"] = "profiles/traffic.csv (ncu --set full, builder-run; not measured by this run)"
@@ -616,6 +651,24 @@ def ours_line(args, cfg, metric, ranks, device, lqcd, torch, full=True):
             line["variants"] = dict(line["variants"] or {}, **{"slab_strong_x%d" % world: sv})
     lat.close()
     return line
+
+
+def config_entry(line):
+    """What the default line's `configs` object keeps of one config's full line (same code, same timing rules)."""
+    e2e, ck = line.get("e2e") or {}, line.get("clocks") or {}
+    out = {"workload": line["config"]["workload"], "cg_path": line["cg"]["path"], "l2_policy": line["config"]["l2_policy"],
+           "steps": line["steps"], "warmup": line["warmup"],
+           "cg_ms": line["ms_per_step"], "iters": line["cg"]["iters"], "true_residual": line["cg"]["true_residual"],
+           "us_per_iteration": line["cg"]["us_per_iteration"], "value_GBps": line["value"],
+           "dslash_us": line["dslash"]["us_per_call"], "dslash_GBps": line["dslash"]["GBps"],
+           "dslash_GFLOPs": line["dslash"]["GFLOPs"], "dslash_frac_of_peak": line["roofline"]["frac"],
+           "dslash_kernel": line["roofline"]["kernel"], "e2e_ms": e2e.get("ms_per_step"),
+           "gpu_launches": line["gpu_launches"], "clocks": ck}
+    if line.get("variants"):
+        out["variants"] = {k: {"time_to_solution_ms": v.get("time_to_solution_ms"), "iters": v.get("iters"),
+                               "reliable_updates": v.get("reliable_updates"), "true_residual": v.get("true_residual"),
+                               "converged": v.get("converged")} for k, v in line["variants"].items()}
+    return out
 
 
 def all_configs_table(lines):
@@ -658,6 +711,8 @@ def main():
     ap.add_argument("--all-configs", action="store_true",
                     help="the five BASELINE.json configs in one run (no variants, no oracle timing): one JSON line with a list")
     ap.add_argument("--table", default=None, help="with --all-configs: also write the five-config table (markdown) to this file")
+    ap.add_argument("--no-configs", action="store_true",
+                    help="N = 1 default line: skip the `configs` object (the other four BASELINE.json configs timed by the same code)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -715,6 +770,22 @@ def main():
         ranks.close()
         return 0
     line = ours_line(args, cfg, metric, ranks, device, lqcd, torch, full=True)
+    if world == 1 and not args.no_configs and args.config == 3 and args.precision == "f64" and args.recon == 18:
+        # north_star: throughput "on all five configs".  The headline (value, roofline, e2e) stays config 3; the other
+        # four are timed here by the same code and rules (>= 3 warm-up solves, args.steps timed solves, device events,
+        # own clock record), each reduced to a few numbers; configs 4 and 5 with their other solvers (even-odd Wilson;
+        # two-row links and mixed precision).  A failure here never takes the headline down.
+        line["configs"] = {}
+        for n in (1, 2, 4, 5):
+            c = synth.config(n)
+            t0 = time.perf_counter()
+            try:
+                entry = config_entry(ours_line(args, c, metric, ranks, device, lqcd, torch, full=False, solver_variants=n in (4, 5)))
+            except Exception as exc:  # noqa: BLE001
+                entry = {"error": repr(exc)[:300]}
+            entry["wall_s_including_input_generation"] = time.perf_counter() - t0
+            line["configs"][c["name"]] = entry
+            torch.cuda.empty_cache()
     if rank == 0:
         print(json.dumps(line))
     ranks.close()

@@ -99,12 +99,20 @@ enum {
      * other modes run with 32-thread blocks (same arithmetic, same summation order: a warp of the
      * cooperative kernel is one 32-thread block of the three-kernel path; 32 is what LQCD_OPT_STAG_BLOCK's
      * automatic choice gives on those lattices); LQCD_OPT_CG_MODE / _CHECK_EVERY do not apply while it is
-     * in use (the exit test runs on the device every iteration). */
+     * in use (the exit test runs on the device every iteration).  The automatic choice never overrides an
+     * explicit lqcd_set_option(LQCD_OPT_CG_MODE, LQCD_CG_SYNC): a caller who asked for the paper's loop with
+     * its host-side exit test gets it on every lattice.  lqcd_last_cg_path() tells which one ran.  A solve
+     * longer than 2^20 iterations continues in further launches of the same kernel (same iterates). */
     LQCD_OPT_PERSISTENT = 5,
     /* Threads per block of the fp64 staggered kernels: 0 (default) = by lattice size (32 / 64 / 128: small
      * lattices are latency-bound and gain from more, smaller blocks), or 32, 64, 128.  Changes how the
      * per-block partial sums are grouped, hence the last bits of the inner products -- nothing else. */
-    LQCD_OPT_STAG_BLOCK = 6
+    LQCD_OPT_STAG_BLOCK = 6,
+    /* Iterations one launch of the LQCD_OPT_PERSISTENT kernel may run, 1..1048576 (default 1048576 = 2^20: the
+     * kernel's grid barrier counts arrivals in 32 bits from zero at launch, three per iteration and block).  A
+     * solve that needs more continues in the next launch from the scalars the last one left on the device,
+     * with one 128-byte read-back in between: same iterates, bit for bit. */
+    LQCD_OPT_PERSISTENT_CHUNK = 7
 };
 
 /* Create a context for an L0 x L1 x L2 x L3 lattice (every extent even and >= 2; L = 2 is
@@ -220,6 +228,13 @@ int lqcd_dslash_host(lqcd_ctx *ctx, int out_parity, const double *in_host, doubl
  * for k <= min(iters, 65535).  Copies at most `capacity` values to rr_host and returns the
  * number copied (negative = error). */
 int lqcd_cg_history(lqcd_ctx *ctx, double *rr_host, int capacity);
+
+/* Which iteration loop the last CG call on this context ran (lqcd_cg_solve, lqcd_cg_solve_mixed,
+ * lqcd_stag_solve_full, lqcd_wilson_solve_eo, lqcd_congrad_host): the host loop in the LQCD_OPT_CG_MODE
+ * form, or the one cooperative kernel of LQCD_OPT_PERSISTENT (where LQCD_OPT_CG_MODE / _CHECK_EVERY played no
+ * part).  LQCD_PATH_NONE before the first solve; LQCD_EARG for a null context.  Host-only. */
+enum { LQCD_PATH_NONE = 0, LQCD_PATH_HOST_LOOP = 1, LQCD_PATH_PERSISTENT = 2 };
+int lqcd_last_cg_path(const lqcd_ctx *ctx);
 
 /* Number of kernels launched by this context since creation (for bench.py's gpu_launches). */
 long long lqcd_kernel_launches(const lqcd_ctx *ctx);

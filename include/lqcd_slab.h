@@ -67,7 +67,7 @@ enum {
     LQCD_SLAB_OPT_GRAPH = 3,        /* 1 (default): when every slab of the call runs on one stream, each batch of
                                        CG iterations is replayed from one CUDA graph (an odd check_every is
                                        rounded up to even); 0: kernel-by-kernel launches.  Same iterates. */
-    LQCD_SLAB_OPT_FUSE_SYNC = 4     /* one-rank-per-process calls only.  1: the last block of every kernel that ends
+    LQCD_SLAB_OPT_FUSE_SYNC = 4,    /* one-rank-per-process calls only.  1: the last block of every kernel that ends
                                        in a sum (the Dslash kernels of the CG, the p-update, the init) also
                                        signals, waits and combines, so an iteration is three launches and the
                                        exchange costs no kernel boundary; 0: a separate small launch per
@@ -75,6 +75,15 @@ enum {
                                        Default: 1 for nranks = 1, 0 for nranks > 1 -- the fused tail has only
                                        ever synchronised with itself (one GPU per box so far); switch it on
                                        explicitly once the separate-launch form has run on real peers. */
+    LQCD_SLAB_OPT_ACQUIRE = 5       /* ordering of a synchronisation point against the ghost faces in the PTX memory
+                                       model.  1: the thread that sends the tagged words first fences at system scope
+                                       (a release of the face stores it learnt of through the ticket chain), and a
+                                       receiver that has seen its words fences at system scope before it goes on (an
+                                       acquire: the next kernel's ghost-face loads cannot see older data).  0: relaxed
+                                       stores and polls only -- enough when every mailbox is in this GPU's memory,
+                                       whose L2 is the point of coherence.  -1 (default): 1 if lqcd_slab_connect found
+                                       a peer mailbox on another device, else 0.  Same iterates; costs two fences
+                                       (microseconds) per synchronisation point, in one block. */
 };
 
 /* Slab of rank `rank` of `nranks` for the global L0 x L1 x L2 x L3 staggered lattice.  L3/nranks must be

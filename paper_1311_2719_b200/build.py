@@ -12,7 +12,7 @@ SO = os.path.join(HERE, "liblqcd_b200.so")
 SOURCES = [os.path.join(CSRC, "lqcd_api.cu"), os.path.join(CSRC, "lqcd_slab.cu"), os.path.join(CSRC, "lqcd_noalloc.cu")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
-    "-O3", "-lineinfo", "-std=c++17",
+    "-O3", "-lineinfo", "-std=c++17", "--threads", "3",   # the three translation units compile side by side
     "-Xcompiler", "-fPIC", "-shared",
     "-I", os.path.join(ROOT, "include"),
 ]

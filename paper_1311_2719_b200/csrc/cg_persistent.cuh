@@ -41,6 +41,10 @@ struct PersistArgs {
     int niter;           // iterations this launch may run
 };
 
+// Link loads of the loop: ordinary L1-allocating loads -- a block re-reads the same links every iteration.  B200, CG ms
+// at cfg 1 / cfg 2 (20 solves, two runs each): streaming (.cs, what the three-kernel path uses) 2.00 / 2.20-2.22,
+// L2 only (.cg) 2.27 / 2.14, default 2.00 / 2.14-2.16 (profiles/r03_bench.md).
+constexpr int kPersistLinks = LP_DEFAULT;
 constexpr int kPersistBlock = 256;   // threads of a physical block = 8 virtual blocks of the hopping terms at a time
 constexpr int kPersistSmemPartials = 2048;
 
@@ -150,10 +154,10 @@ __global__ void __launch_bounds__(kPersistBlock, 1) stag_cg_persistent_kernel(co
             if (e < a.g.Vh) {
                 cplx acc[3] = { czero<cplx>(), czero<cplx>(), czero<cplx>() };
                 const Site s = decode_site(a.g, 1, e);
-                stag_hop<0, RECON, false, cplx, VL_PLAIN>(d1, s, acc);
-                stag_hop<1, RECON, false, cplx, VL_PLAIN>(d1, s, acc);
-                stag_hop<2, RECON, false, cplx, VL_PLAIN>(d1, s, acc);
-                stag_hop<3, RECON, false, cplx, VL_PLAIN>(d1, s, acc);
+                stag_hop<0, RECON, false, cplx, VL_PLAIN, kPersistLinks>(d1, s, acc);
+                stag_hop<1, RECON, false, cplx, VL_PLAIN, kPersistLinks>(d1, s, acc);
+                stag_hop<2, RECON, false, cplx, VL_PLAIN, kPersistLinks>(d1, s, acc);
+                stag_hop<3, RECON, false, cplx, VL_PLAIN, kPersistLinks>(d1, s, acc);
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
                     st_vec(a.t + c * Vh + e, acc[c]);
@@ -175,10 +179,10 @@ __global__ void __launch_bounds__(kPersistBlock, 1) stag_cg_persistent_kernel(co
             if (e < a.g.Vh) {
                 cplx acc[3] = { czero<cplx>(), czero<cplx>(), czero<cplx>() };
                 const Site s = decode_site(a.g, 0, e);
-                stag_hop<0, RECON, false, cplx, VL_PLAIN>(d2, s, acc);
-                stag_hop<1, RECON, false, cplx, VL_PLAIN>(d2, s, acc);
-                stag_hop<2, RECON, false, cplx, VL_PLAIN>(d2, s, acc);
-                stag_hop<3, RECON, false, cplx, VL_PLAIN>(d2, s, acc);
+                stag_hop<0, RECON, false, cplx, VL_PLAIN, kPersistLinks>(d2, s, acc);
+                stag_hop<1, RECON, false, cplx, VL_PLAIN, kPersistLinks>(d2, s, acc);
+                stag_hop<2, RECON, false, cplx, VL_PLAIN, kPersistLinks>(d2, s, acc);
+                stag_hop<3, RECON, false, cplx, VL_PLAIN, kPersistLinks>(d2, s, acc);
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
                     const size_t i = c * Vh + e;

@@ -101,22 +101,16 @@ __device__ __forceinline__ float2 ld_stream(const float2* p)
 // Link loads by cache policy.  LP_STREAM: as above (fields larger than L2).  LP_L2: through L2 with normal
 // eviction and no L1 allocation -- for fields that FIT in L2 and are read by both parities of a full-lattice
 // operator (each link is the forward link of x and the backward link of x+mu^), so the second use and every
-// later iteration hits L2.  LP_L2_LAST: the same, marked evict-last.
-enum LinkPolicy { LP_STREAM = 0, LP_L2 = 1, LP_L2_LAST = 2, LP_DEFAULT = 3 };
-__device__ __forceinline__ unsigned long long l2_evict_last_policy()
-{
-    unsigned long long pol;
-    asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
-    return pol;
-}
+// later iteration hits L2.  LP_DEFAULT: ordinary loads that also allocate in L1 -- for the one-kernel CG loop
+// (cg_persistent.cuh), whose links are re-read by the same block every iteration.  (An evict-last L2 policy
+// and a persisting-L2 window were measured and dropped: DESIGN.md.)
+enum LinkPolicy { LP_STREAM = 0, LP_L2 = 1, LP_DEFAULT = 2 };
 template <int POLICY>
 __device__ __forceinline__ double2 ld_link(const double2* p)
 {
     double2 v;
     if (POLICY == LP_L2)
         asm volatile("ld.global.cg.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
-    else if (POLICY == LP_L2_LAST)
-        asm volatile("ld.global.L1::no_allocate.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(l2_evict_last_policy()));
     else if (POLICY == LP_DEFAULT)
         asm volatile("ld.global.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
     else
@@ -129,8 +123,6 @@ __device__ __forceinline__ float2 ld_link(const float2* p)
     float2 v;
     if (POLICY == LP_L2)
         asm volatile("ld.global.cg.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
-    else if (POLICY == LP_L2_LAST)
-        asm volatile("ld.global.L1::no_allocate.L2::cache_hint.v2.f32 {%0, %1}, [%2], %3;" : "=f"(v.x), "=f"(v.y) : "l"(p), "l"(l2_evict_last_policy()));
     else if (POLICY == LP_DEFAULT)
         asm volatile("ld.global.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
     else
@@ -152,8 +144,6 @@ __device__ __forceinline__ C ld_vec(const C* p)
 }
 template <class C>
 __device__ __forceinline__ void st_vec(C* p, C v) { *p = v; }
-// Ask L2 for the 128-byte line of p; nothing is returned and no register waits for it.
-__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 // x is read and written exactly once per CG iteration: stream it past the caches.
 __device__ __forceinline__ void st_stream(double2* p, double2 v)
 {
@@ -169,7 +159,6 @@ __device__ __forceinline__ double2 cmake(double re, double im) { return make_dou
 __device__ __forceinline__ float2 cmake(float re, float im) { return make_float2(re, im); }
 template <class C> __device__ __forceinline__ C czero() { C z; z.x = 0; z.y = 0; return z; }
 template <class C> __device__ __forceinline__ C cadd(C a, C b) { return cmake(a.x + b.x, a.y + b.y); }
-template <class C> __device__ __forceinline__ C csub(C a, C b) { return cmake(a.x - b.x, a.y - b.y); }
 __device__ __forceinline__ double2 cscale(double s, double2 a) { return cmake(s * a.x, s * a.y); }
 __device__ __forceinline__ float2 cscale(double s, float2 a) { return cmake((float)s * a.x, (float)s * a.y); }
 // |a|^2, always returned (and summed by the caller) in fp64

@@ -64,6 +64,10 @@ struct lqcd_ctx {
     int f32_pairs;          // fp32 kernels of the mixed solver: two sites per thread with 128-bit loads
     int stag_block;         // 0 auto (stag_block_for), or 32 / 64 / 128 threads per block of the fp64 staggered kernels
     int persistent;         // -1 auto, 0 never, 1 always: the CG loop as one cooperative kernel (cg_persistent.cuh)
+    bool cg_mode_set;       // LQCD_OPT_CG_MODE was set by the caller: the automatic choice above then respects LQCD_CG_SYNC
+    int last_path;          // LQCD_PATH_* of the last lqcd_cg_solve-type call (lqcd_last_cg_path)
+    int persist_chunk;      // LQCD_OPT_PERSISTENT_CHUNK: iterations per launch of the cooperative kernel
+    int nsm;                // multiprocessors of the device the workspace was bound on (148 on B200 until then)
     bool links_fit_l2;  // the stored link field is at most a third of the L2 (set by lqcd_load_gauge)
     bool wilson_eo;  // set while lqcd_wilson_solve_eo runs: the CG works on Mhat^+ Mhat, even half of the vectors
     // host side
@@ -150,7 +154,8 @@ VecLayout vec_layout(const lqcd_ctx* ctx)
 unsigned int vec_grid(const lqcd_ctx* ctx)
 {
     size_t b = (vec_layout(ctx).n + kVecBlock - 1) / kVecBlock;
-    const size_t cap = 148 * 8;
+    size_t cap = (size_t)ctx->nsm * 8;   // eight 256-thread blocks per multiprocessor: one wave of the vector kernels
+    if (cap > 4096) cap = 4096;          // the partial-sum area has V/32 + 4096 slots (lqcd_create)
     if (b > cap) b = cap;
     if (b < 1) b = 1;
     return (unsigned int)b;
@@ -180,8 +185,8 @@ int stag_block_for(const lqcd_ctx* ctx)
 {
     if (ctx->stag_block) return ctx->stag_block;  // LQCD_OPT_STAG_BLOCK
     const long long blocks128 = ((long long)ctx->g.Vh + 127) / 128;
-    if (blocks128 < 2 * 148) return 32;
-    if (blocks128 < 8 * 148) return 64;
+    if (blocks128 < 2 * ctx->nsm) return 32;
+    if (blocks128 < 8 * ctx->nsm) return 64;
     return 128;
 }
 
@@ -402,8 +407,16 @@ bool use_persistent(const lqcd_ctx* ctx)
 {
     if (ctx->fermion != LQCD_STAGGERED || ctx->wilson_eo) return false;
     if (ctx->persistent >= 0) return ctx->persistent == 1;
+    // automatic: never against an explicit request for the paper's loop with its host-side exit test
+    if (ctx->cg_mode_set && ctx->cg_mode == LQCD_CG_SYNC) return false;
     return ctx->links_fit_l2;
 }
+
+// Iterations one launch of the cooperative kernel may run.  Its grid barrier counts arrivals in 32 bits from
+// zero at launch: three barriers per iteration and at most one block per multiprocessor, so 2^20 iterations
+// stay far below 2^32 arrivals (3 * 2^20 * 1024 blocks = 2^31.6); longer solves continue in a fresh launch
+// (the scalars round-trip through CgScalars, the iterates do not change).
+constexpr int kPersistChunk = 1 << 20;
 
 template <int RECON>
 int launch_persistent_recon(lqcd_ctx* ctx, double mass, cplx* x, int niter)
@@ -459,15 +472,22 @@ int cg_run(lqcd_ctx* ctx, double mass_or_kappa, double tol, int maxiter, const c
     LQCD_LAUNCH_CHECK();
 
     CgScalars* h = ctx->h_sc;
+    ctx->last_path = LQCD_PATH_HOST_LOOP;
     if (use_persistent(ctx)) {
         // one launch runs the loop to the exit rule (or maxiter); the scalars come back once
-        if (maxiter > 0) {
-            rc = launch_persistent(ctx, mass_or_kappa, x, maxiter);
+        ctx->last_path = LQCD_PATH_PERSISTENT;
+        int left = maxiter > 0 ? maxiter : 0;
+        do {
+            const int chunk = left < ctx->persist_chunk ? left : ctx->persist_chunk;
+            if (chunk > 0) {
+                rc = launch_persistent(ctx, mass_or_kappa, x, chunk);
+                if (rc) return rc;
+            }
+            left -= chunk;
+            rc = read_scalars(ctx, 0);
             if (rc) return rc;
-        }
-        rc = read_scalars(ctx, 0);
-        if (rc) return rc;
-        LQCD_CUDA(cudaEventSynchronize(ctx->ev[0]));
+            LQCD_CUDA(cudaEventSynchronize(ctx->ev[0]));
+        } while (left > 0 && !h[0].done);
     } else if (ctx->cg_mode == LQCD_CG_SYNC) {
         // The paper's loop: one scalar comes back per iteration, the exit test runs on the host
         // (PAPER.md:75-76, :91-93, :100).
@@ -604,9 +624,10 @@ int mixed_reliable_update(lqcd_ctx* ctx, double mass, const cplx* b, cplx* x)
 int cg_run_mixed(lqcd_ctx* ctx, double mass, double tol, double delta, int maxiter, const cplx* b, cplx* x)
 {
     int rc;
+    ctx->last_path = LQCD_PATH_HOST_LOOP;
     if (!ctx->gauge_f_ready) {
         const size_t n = (size_t)ctx->g.V * 4 * (size_t)(ctx->recon / 2);
-        gauge_narrow_kernel<<<148 * 8, 256, 0, ctx->stream>>>(ctx->gauge(), ctx->gauge_f(), n);
+        gauge_narrow_kernel<<<ctx->nsm * 8, 256, 0, ctx->stream>>>(ctx->gauge(), ctx->gauge_f(), n);
         LQCD_LAUNCH_CHECK();
         ctx->gauge_f_ready = true;
     }
@@ -707,6 +728,10 @@ int lqcd_create(lqcd_ctx** out, int L0, int L1, int L2, int L3, int fermion_type
     c->congrad_precision = 64;
     c->f32_pairs = 1;
     c->persistent = -1;
+    c->cg_mode_set = false;
+    c->persist_chunk = kPersistChunk;
+    c->last_path = LQCD_PATH_NONE;
+    c->nsm = 148;
 
     size_t off = 0;
     const size_t vec_bytes = align_up(c->nvec * sizeof(cplx));
@@ -765,6 +790,10 @@ int lqcd_set_workspace(lqcd_ctx* ctx, void* workspace_dev, size_t bytes, void* c
     if (ndev < 1) return fail(ctx, LQCD_ECUDA, "no CUDA device");
     int rc = ensure_host(ctx);
     if (rc) return rc;
+    int dev = 0, nsm = 0;
+    LQCD_CUDA(cudaGetDevice(&dev));
+    LQCD_CUDA(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+    if (nsm > 0) ctx->nsm = nsm;
     ctx->ws = (char*)workspace_dev;
     ctx->stream = (cudaStream_t)cuda_stream;
     ctx->gauge_loaded = false;
@@ -779,6 +808,7 @@ int lqcd_set_option(lqcd_ctx* ctx, int option, int value)
     if (option == LQCD_OPT_CG_MODE) {
         if (value < LQCD_CG_SYNC || value > LQCD_CG_GRAPH) return fail(ctx, LQCD_EARG, "bad CG mode %d", value);
         ctx->cg_mode = value;
+        ctx->cg_mode_set = true;
         return LQCD_OK;
     }
     if (option == LQCD_OPT_CG_CHECK_EVERY) {
@@ -806,6 +836,11 @@ int lqcd_set_option(lqcd_ctx* ctx, int option, int value)
     if (option == LQCD_OPT_STAG_BLOCK) {
         if (value != 0 && value != 32 && value != 64 && value != 128) return fail(ctx, LQCD_EARG, "stag_block must be 0 (auto), 32, 64 or 128");
         ctx->stag_block = value;
+        return LQCD_OK;
+    }
+    if (option == LQCD_OPT_PERSISTENT_CHUNK) {
+        if (value < 1 || value > kPersistChunk) return fail(ctx, LQCD_EARG, "persistent chunk must be in 1..%d", kPersistChunk);
+        ctx->persist_chunk = value;
         return LQCD_OK;
     }
     if (option == LQCD_OPT_PERSISTENT) {
@@ -1162,6 +1197,8 @@ int lqcd_cg_history(lqcd_ctx* ctx, double* rr_host, int capacity)
 }
 
 long long lqcd_kernel_launches(const lqcd_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int lqcd_last_cg_path(const lqcd_ctx* ctx) { return ctx ? ctx->last_path : LQCD_EARG; }
 
 const char* lqcd_last_error(const lqcd_ctx* ctx) { return ctx ? ctx->err : "null context"; }
 

@@ -36,6 +36,7 @@ struct lqcd_slab {
     // mailbox (peer-visible) byte offsets
     size_t mb_word, mb_ghost, mb_needed;
     size_t max_blocks;
+    int nsm;      // multiprocessors of the device the memory was bound on (148 on B200 until then)
     char* ws;
     char* mb;
     char* peer[LQCD_SLAB_MAX_RANKS];
@@ -44,6 +45,8 @@ struct lqcd_slab {
     bool memory_set, connected, gauge_loaded;
     bool gauge_f_ready;  // the fp32 link copies match the loaded fp64 ones
     int recon, check_every, timeout_ms, use_graph, fuse_sync;
+    int acquire;       // LQCD_SLAB_OPT_ACQUIRE: -1 auto (= peers_remote), 0, 1
+    bool peers_remote;  // some peer's mailbox is on another device (set by lqcd_slab_connect)
     unsigned long long seq;  // synchronisation points passed
     CgScalars* h_sc;         // pinned, 2 slots
     SlabScalars* h_ss;       // pinned
@@ -113,7 +116,8 @@ int fail(lqcd_slab* s, int code, const char* fmt, ...)
 unsigned int vec_grid(const lqcd_slab* s)
 {
     size_t b = (s->nvec + kVecBlock - 1) / kVecBlock;
-    const size_t cap = 148 * 8;
+    size_t cap = (size_t)s->nsm * 8;
+    if (cap > 4096) cap = 4096;   // the partial-sum area has V/64 + 4096 slots
     if (b > cap) b = cap;
     if (b < 1) b = 1;
     return (unsigned int)b;
@@ -221,8 +225,8 @@ StagArgsD stag_args(const lqcd_slab* s, int parity, const cplx* in, cplx* out, b
 int slab_block_for(const lqcd_slab* s)
 {
     const long long blocks128 = ((long long)s->g.Vh + 127) / 128;
-    if (blocks128 < 2 * 148) return 32;
-    if (blocks128 < 8 * 148) return 64;
+    if (blocks128 < 2 * s->nsm) return 32;
+    if (blocks128 < 8 * s->nsm) return 64;
     return 128;
 }
 
@@ -294,6 +298,7 @@ SlabSyncArgs sync_args(const lqcd_slab* s, int op, int nvals, double m2, double 
     a.delta = delta;
     a.maxiter = maxiter;
     a.timeout_ns = (unsigned long long)s->timeout_ms * 1000000ull;
+    a.sys_fences = s->acquire >= 0 ? s->acquire : (s->peers_remote ? 1 : 0);
     return a;
 }
 
@@ -673,7 +678,7 @@ int ensure_gauge_f(lqcd_slab* s)
 {
     if (s->gauge_f_ready) return LQCD_OK;
     const size_t nc = (size_t)(s->recon / 2);
-    gauge_narrow_kernel<<<148 * 8, 256, 0, s->stream>>>(s->gauge(), s->gauge_f(), (size_t)s->g.V * 4 * nc);
+    gauge_narrow_kernel<<<s->nsm * 8, 256, 0, s->stream>>>(s->gauge(), s->gauge_f(), (size_t)s->g.V * 4 * nc);
     SLAB_LAUNCH_CHECK();
     gauge_narrow_kernel<<<64, 256, 0, s->stream>>>(s->gghost(), s->gghost_f(), 2 * nc * (size_t)s->sh);
     SLAB_LAUNCH_CHECK();
@@ -888,11 +893,13 @@ int lqcd_slab_create(lqcd_slab** out, int L0, int L1, int L2, int L3, int rank, 
     c->sh = c->g.s3;
     c->nvec = 3 * (size_t)(V / 2);
     c->max_blocks = (size_t)V / 64 + 4096;
+    c->nsm = 148;
     c->recon = 18;
     c->check_every = 8;
     c->timeout_ms = 20000;
     c->use_graph = 1;
     c->fuse_sync = nranks == 1 ? 1 : 0;  // see LQCD_SLAB_OPT_FUSE_SYNC: unvalidated across GPUs
+    c->acquire = -1;
 
     size_t off = 0;
     const size_t vec_bytes = align_up(c->nvec * sizeof(cplx));
@@ -960,6 +967,9 @@ int lqcd_slab_set_memory(lqcd_slab* s, void* workspace_dev, size_t workspace_byt
     SLAB_CUDA(cudaSetDevice(s->device));
     int rc = ensure_host(s);
     if (rc) return rc;
+    int nsm = 0;
+    SLAB_CUDA(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, s->device));
+    if (nsm > 0) s->nsm = nsm;
     s->ws = (char*)workspace_dev;
     s->mb = (char*)mailbox_dev;
     s->stream = (cudaStream_t)cuda_stream;
@@ -982,6 +992,15 @@ int lqcd_slab_connect(lqcd_slab* s, void* const* peer_mailboxes)
     for (int r = 0; r < s->nranks; ++r)
         if (!peer_mailboxes[r]) return fail(s, LQCD_EARG, "mailbox of rank %d is null", r);
     if (peer_mailboxes[s->rank] != (void*)s->mb) return fail(s, LQCD_EARG, "peer_mailboxes[rank] must be the own mailbox");
+    // Which device holds each peer's mailbox?  One on another GPU switches the system-scope release / acquire of the
+    // synchronisation points on (slab_sync.cuh).  A pointer the runtime cannot place is treated as remote.
+    s->peers_remote = false;
+    for (int r = 0; r < s->nranks; ++r) {
+        cudaPointerAttributes at;
+        const cudaError_t e = cudaPointerGetAttributes(&at, peer_mailboxes[r]);
+        if (e != cudaSuccess) (void)cudaGetLastError();
+        if (e != cudaSuccess || at.type != cudaMemoryTypeDevice || at.device != s->device) s->peers_remote = true;
+    }
     for (int r = 0; r < s->nranks; ++r) s->peer[r] = (char*)peer_mailboxes[r];
     s->connected = true;
     return LQCD_OK;
@@ -1009,6 +1028,11 @@ int lqcd_slab_set_option(lqcd_slab* s, int option, int value)
     if (option == LQCD_SLAB_OPT_FUSE_SYNC) {
         if (value != 0 && value != 1) return fail(s, LQCD_EARG, "fuse_sync must be 0 or 1");
         s->fuse_sync = value;
+        return LQCD_OK;
+    }
+    if (option == LQCD_SLAB_OPT_ACQUIRE) {
+        if (value < -1 || value > 1) return fail(s, LQCD_EARG, "acquire must be -1 (auto), 0 or 1");
+        s->acquire = value;
         return LQCD_OK;
     }
     if (option == LQCD_SLAB_OPT_GRAPH) {

@@ -58,6 +58,7 @@ struct SlabSyncArgs {
     double m2, tol, delta;
     int maxiter;
     unsigned long long timeout_ns;
+    int sys_fences;   // 1: a peer's mailbox is on another GPU (LQCD_SLAB_OPT_ACQUIRE): release before the words, acquire after
 };
 
 __device__ __forceinline__ void st_sys_u64(unsigned long long* p, unsigned long long v)
@@ -73,11 +74,21 @@ __device__ __forceinline__ unsigned long long ld_relaxed_sys_u64(const unsigned 
     return v;
 }
 
+__device__ __forceinline__ void fence_acq_rel_sys() { asm volatile("fence.acq_rel.sys;" ::: "memory"); }
+
 // thread r < nranks: this rank's partial(s), tagged with the number of the synchronisation point, into rank r's
 // mailbox.  The faces were stored -- and fenced at system scope -- by the producer's blocks before this runs.
 // own: the partial(s) in registers (fused tail), or null = read them from `part` (left there by the producer kernel).
+//
+// Memory model, sender side.  The face stores were made by OTHER blocks (each fenced them at system scope before
+// its ticket atomic); this thread learnt of them through the ticket chain, which is ordered at DEVICE scope only
+// (__threadfence in grid_sum_block's last block).  With every mailbox on this GPU that is the same thing.  With a
+// peer on another GPU the words must not become visible THERE before the faces: a system-scope fence between
+// "observed the last ticket" and "store the words" makes the chain cumulative at system scope (fence + relaxed
+// store = a release of everything this thread has observed).  One fence in at most 16 threads of one block.
 __device__ __forceinline__ void slab_signal(const SlabSyncArgs& a, unsigned long long seq, int r, const double* own = nullptr)
 {
+    if (a.sys_fences) fence_acq_rel_sys();
     unsigned long long* dst = a.peer_word[r] + ((seq & 1ull) * a.nranks + a.rank) * 4;
     const unsigned long long tag = seq << 32;
     const int nv = a.nvals > 0 ? a.nvals : 1;  // a point without a sum still announces itself
@@ -116,6 +127,12 @@ __device__ __forceinline__ bool slab_wait(const SlabSyncArgs& a, unsigned long l
         }
         val[k] = __longlong_as_double((long long)((hi << 32) | (lo & 0xffffffffull)));
     }
+    // Receiver side.  The sums need no ordering (the data is the word).  The ghost faces the words announce are read
+    // by the NEXT kernel of this stream; that the peer's face stores are visible to it rests, without a fence, on this
+    // GPU's L2 being the point of coherence of its own memory.  With a peer on another GPU the relaxed poll is followed
+    // by a system-scope fence (relaxed load + fence = acquire), which pairs with the sender's release above; the kernel
+    // boundary then carries the order to the next kernel's loads.
+    if (a.sys_fences) fence_acq_rel_sys();
     return true;
 }
 

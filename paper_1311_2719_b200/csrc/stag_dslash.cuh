@@ -70,7 +70,8 @@ struct StagArgs {
     SlabArgs<C> sl;  // used by the SLAB instantiations only
 };
 
-template <int MU, int RECON, bool SLAB, class C, int VL = VL_NC>
+// LINKS: cache policy of the link loads of the undivided lattice (device_common.cuh LinkPolicy).
+template <int MU, int RECON, bool SLAB, class C, int VL = VL_NC, int LINKS = LP_STREAM>
 __device__ __forceinline__ void stag_hop(const StagArgs<C>& a, const Site& s, C acc[3])
 {
     constexpr int NC = RECON / 2;
@@ -106,10 +107,10 @@ __device__ __forceinline__ void stag_hop(const StagArgs<C>& a, const Site& s, C 
         const int ef = nbr_fwd<MU>(a.g, s);
         const int eb = nbr_bwd<MU>(a.g, s);
         const C* Ub = a.gauge + (size_t)(((1 - a.parity) * 4 + MU) * NC) * Vh + eb;
-        load_link<RECON>(Uf, Vh, U);
+        load_link<RECON, C, LINKS>(Uf, Vh, U);
 #pragma unroll
         for (int c = 0; c < 3; ++c) vf[c] = ld_vec<VL>(a.in + c * Vh + ef);
-        load_link<RECON>(Ub, Vh, W);
+        load_link<RECON, C, LINKS>(Ub, Vh, W);
 #pragma unroll
         for (int c = 0; c < 3; ++c) vb[c] = ld_vec<VL>(a.in + c * Vh + eb);
         sf = eta * bc_fwd<MU>(a.g, s);

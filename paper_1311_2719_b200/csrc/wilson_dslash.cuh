@@ -29,9 +29,6 @@
 #ifndef LQCD_WILSON_EPI_BATCH_U
 #define LQCD_WILSON_EPI_BATCH_U 6
 #endif
-#ifndef LQCD_WILSON_PREFETCH
-#define LQCD_WILSON_PREFETCH 0
-#endif
 
 namespace lqcd {
 
@@ -342,16 +339,6 @@ __global__ void __launch_bounds__(BLOCK, LQCD_WILSON_MINB) wilson_dslash_kernel(
     for (int s = 0; s < 4; ++s)
 #pragma unroll
         for (int c = 0; c < 3; ++c) acc[s][c] = czero<cplx>();
-#if LQCD_WILSON_PREFETCH
-    // The residual at the own site is first needed after the eight hops: ask L2 for its lines now (one request
-    // per 128-byte line, no register held), so that the epilogue's loads find them there.
-    if (EPI == WE_CGUPDATE || EPI == WE_EO_CGUPDATE) {
-        if (active && (threadIdx.x & 7) == 0) {
-#pragma unroll
-            for (int k = 0; k < 12; ++k) prefetch_l2(a.r + (size_t)k * a.g.V + gsite);
-        }
-    }
-#endif
     constexpr int VL = wilson_one_parity(EPI) ? VL_PLAIN : VL_NC;
     if (active) {
         const Site st = decode_site(a.g, parity, e);

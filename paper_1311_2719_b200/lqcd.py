@@ -20,7 +20,9 @@ STAGGERED, WILSON = 0, 1
 EVEN, ODD = 0, 1
 OK, MAXITER = 0, 1
 CG_SYNC, CG_ASYNC, CG_GRAPH = 0, 1, 2
+PATH_NONE, PATH_HOST_LOOP, PATH_PERSISTENT = 0, 1, 2
 OPT_CG_MODE, OPT_CG_CHECK_EVERY, OPT_RECONSTRUCT, OPT_CONGRAD_PRECISION, OPT_F32_PAIRS, OPT_PERSISTENT, OPT_STAG_BLOCK = 0, 1, 2, 3, 4, 5, 6
+OPT_PERSISTENT_CHUNK = 7
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _ROOT = os.path.dirname(_HERE)
@@ -78,6 +80,7 @@ def load_library():
     L.lqcd_cg_history.argtypes = [P, P, I]
     L.lqcd_kernel_launches.argtypes = [P]
     L.lqcd_kernel_launches.restype = ctypes.c_longlong
+    L.lqcd_last_cg_path.argtypes = [P]
     L.lqcd_last_error.argtypes = [P]
     L.lqcd_last_error.restype = ctypes.c_char_p
     _lib = L
@@ -176,6 +179,10 @@ class Lattice:
 
     def kernel_launches(self) -> int:
         return int(self._lib.lqcd_kernel_launches(self._ctx))
+
+    def last_cg_path(self) -> int:
+        """PATH_NONE / PATH_HOST_LOOP / PATH_PERSISTENT: the iteration loop the last CG call ran."""
+        return int(self._lib.lqcd_last_cg_path(self._ctx))
 
     # ------------------------------------------------------------------ the calls of include/lqcd.h
     def load_gauge(self, u: torch.Tensor):

@@ -24,7 +24,7 @@ from .lqcd import EVEN, ODD, LqcdError  # noqa: F401
 
 ECOMM = -6
 MAX_RANKS = 16
-OPT_RECONSTRUCT, OPT_CHECK_EVERY, OPT_TIMEOUT_MS, OPT_GRAPH, OPT_FUSE_SYNC = 0, 1, 2, 3, 4
+OPT_RECONSTRUCT, OPT_CHECK_EVERY, OPT_TIMEOUT_MS, OPT_GRAPH, OPT_FUSE_SYNC, OPT_ACQUIRE = 0, 1, 2, 3, 4, 5
 
 _HEADER = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "include", "lqcd_slab.h")
 

@@ -213,6 +213,61 @@ def test_cg_persistent_kernel_changes_no_bit(lq, dims, recon, every):
     assert abs(p[1] - want["iters"]) <= 2 and rel(p[0], want["x"]) <= CG_TOL
 
 
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (10, 6, 6, 4)])
+def test_cg_persistent_kernel_in_several_launches_changes_no_bit(lq, dims):
+    """LQCD_OPT_PERSISTENT_CHUNK: the one-kernel loop cut into launches of 7 iterations (what a solve longer than
+    2^20 iterations does, so that the 32-bit arrival counter of the grid barrier cannot wrap) continues from the
+    scalars the previous launch left on the device: same iterates, count, history and residual as ONE launch,
+    and the number of launches is what the chunking says."""
+    mass = 0.05
+    u = synth.gauge_field(dims, "haar", 33)
+    b = synth.source(dims, "staggered", 34)
+    got = {}
+    with make_lattice(lq, dims, 0, u) as lat:
+        lat.set_option(lq.OPT_PERSISTENT, 1)
+        for chunk in (1 << 20, 7):
+            lat.set_option(lq.OPT_PERSISTENT_CHUNK, chunk)
+            n0 = lat.kernel_launches()
+            x, it, res, status = lat.cg_solve(mass, 1e-10, 20000, dev(b))
+            assert lat.last_cg_path() == lq.PATH_PERSISTENT
+            got[chunk] = (host(x), it, res, status, lat.cg_history().numpy(), lat.kernel_launches() - n0)
+            xk, itk, _, stk = lat.cg_solve(mass, 0.0, 15, dev(b))      # tol = 0: exactly 15 = 7 + 7 + 1 iterations
+            got[chunk] += (host(xk), itk, stk)
+        with pytest.raises(lq.LqcdError):
+            lat.set_option(lq.OPT_PERSISTENT_CHUNK, 0)
+    one, cut = got[1 << 20], got[7]
+    assert one[3] == cut[3] == 0 and one[1] == cut[1] and one[2] == cut[2]
+    assert np.array_equal(one[0], cut[0]) and np.array_equal(one[4], cut[4])
+    assert one[5] == 4 and cut[5] == 3 + (cut[1] + 6) // 7        # init + loop launches + the two kernels of the final check
+    assert one[7] == cut[7] == 15 and one[8] == cut[8] == 1 and np.array_equal(one[6], cut[6])
+
+
+def test_automatic_one_kernel_loop_respects_an_explicit_host_side_exit_test(lq):
+    """On a lattice whose links fit the L2 the default (LQCD_OPT_PERSISTENT = -1) picks the one-kernel loop -- but not
+    over a caller who set LQCD_CG_SYNC, the paper's loop with the exit test on the host (PAPER.md:91-93, :100);
+    lqcd_last_cg_path says which loop ran.  The iterates are the same bits either way."""
+    dims, mass = (4, 4, 4, 4), 0.1
+    u = synth.gauge_field(dims, "haar", 35)
+    b = synth.source(dims, "staggered", 36)
+    with make_lattice(lq, dims, 0, u) as lat:
+        assert lat.last_cg_path() == lq.PATH_NONE
+        x0, it0, res0, st0 = lat.cg_solve(mass, 1e-10, 5000, dev(b))
+        assert lat.last_cg_path() == lq.PATH_PERSISTENT                      # automatic, nothing set
+        lat.set_option(lq.OPT_CG_MODE, lq.CG_GRAPH)
+        lat.cg_solve(mass, 1e-10, 5000, dev(b))
+        assert lat.last_cg_path() == lq.PATH_PERSISTENT                      # GRAPH / ASYNC leave the choice automatic
+        lat.set_option(lq.OPT_CG_MODE, lq.CG_SYNC)
+        n0 = lat.kernel_launches()
+        x1, it1, res1, st1 = lat.cg_solve(mass, 1e-10, 5000, dev(b))
+        assert lat.last_cg_path() == lq.PATH_HOST_LOOP and lat.kernel_launches() - n0 >= 3 * it1
+        assert (it0, res0, st0) == (it1, res1, st1) and torch.equal(x0, x1)
+        lat.set_option(lq.OPT_PERSISTENT, 1)                                 # an explicit 1 still wins
+        lat.cg_solve(mass, 1e-10, 5000, dev(b))
+        assert lat.last_cg_path() == lq.PATH_PERSISTENT
+        lat.cg_solve_mixed(mass, 1e-10, 5000, dev(b))
+        assert lat.last_cg_path() == lq.PATH_HOST_LOOP
+
+
 @pytest.mark.parametrize("dims", [(4, 4, 4, 4), (6, 4, 2, 2), (8, 8, 8, 4)])
 def test_wilson_cg_modes_and_the_x_update_in_the_vector_kernel(lq, dims):
     """The Wilson CG does x += alpha p in the vector kernel that follows the update of r (cg_xpupdate_kernel).  The

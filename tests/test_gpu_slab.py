@@ -240,6 +240,33 @@ def test_slab_fused_synchronisation_changes_no_bit(sl):
         g.close()
 
 
+def test_slab_system_scope_release_acquire_changes_no_bit(sl):
+    """LQCD_SLAB_OPT_ACQUIRE = 1 (the fences a peer on another GPU gets by default) forced on one GPU: the ring of one
+    rank with the fused tail and with separate launches, same bits as without; automatic = off here (the
+    mailbox is on the same device), and the option rejects other values."""
+    c, u, b = synth.config_inputs(1)
+    dims = c["dims"]
+    ug = torch.from_numpy(u)
+    s = sl.Slab(dims, 0, 1)
+    try:
+        s.connect([s.mailbox_ptr])
+        s.load_gauge(sl.local_gauge(ug, dims, 0, 1).cuda(), sl.u3_below_from_global(ug, dims, 0, 1).cuda())
+        got = []
+        for acquire, fuse in ((-1, 1), (1, 1), (1, 0), (0, 0)):
+            s.set_option(sl.OPT_ACQUIRE, acquire)
+            s.set_option(sl.OPT_FUSE_SYNC, fuse)
+            x, it, res, status = s.cg_solve(c["param"], c["tol"], 20000, torch.from_numpy(b).cuda(), s.new_vector())
+            got.append((x.cpu().numpy(), it, res, status))
+        for x, it, res, status in got[1:]:
+            assert status == 0 and it == got[0][1] and res == got[0][2] and np.array_equal(x, got[0][0])
+        want = oracle.cg(dims, 0, u, c["param"], c["tol"], 20000, b)
+        assert abs(got[0][1] - want["iters"]) <= 2 and rel(got[0][0], want["x"]) <= CG_TOL
+        with pytest.raises(Exception):
+            s.set_option(sl.OPT_ACQUIRE, 2)
+    finally:
+        s.close()
+
+
 def test_slab_edge_cases_and_errors(sl):
     c, u, b = synth.config_inputs(1)
     dims = c["dims"]
@@ -506,7 +533,7 @@ def test_slab_ipc_mailboxes_between_two_processes():
 
 
 # ------------------------------------------------------------------ two GPUs, one process each (runs only where two are visible)
-def _two_gpu_worker(rank, world, port, fuse, out):
+def _two_gpu_worker(rank, world, port, fuse, acquire, out):
     """One rank per process and per GPU: IPC-mapped mailboxes, face stores and flags over NVLink, compute calls on
     both sides -- the configuration a one-GPU box cannot run (two kernels that wait on one another must not
     share a GPU).  Each rank reports its slab of D b, A b and the CG solution; the parent compares the
@@ -529,6 +556,7 @@ def _two_gpu_worker(rank, world, port, fuse, out):
         s = sl.Slab(dims, rank, world, device=dev)
         s.set_option(sl.OPT_TIMEOUT_MS, 5000)
         s.set_option(sl.OPT_FUSE_SYNC, fuse)
+        s.set_option(sl.OPT_ACQUIRE, acquire)
         s.connect_ipc()
         ul = sl.local_gauge(u, dims, rank, world)
         ub = sl.exchange_u3_below(ul, dims, rank, world)      # the set-up exchange over torch.distributed
@@ -549,8 +577,9 @@ def _two_gpu_worker(rank, world, port, fuse, out):
     dist.destroy_process_group()
 
 
+@pytest.mark.parametrize("acquire", [-1, 1, 0])   # -1: automatic (on: the peer is another GPU); 0: relaxed words only
 @pytest.mark.parametrize("fuse", [0, 1])
-def test_slab_two_gpus_one_process_each(fuse):
+def test_slab_two_gpus_one_process_each(fuse, acquire):
     import socket
     import torch.multiprocessing as mp
     if torch.cuda.device_count() < 2:
@@ -563,7 +592,7 @@ def test_slab_two_gpus_one_process_each(fuse):
     sock.close()
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
-    procs = [ctx.Process(target=_two_gpu_worker, args=(i, 2, port, fuse, q)) for i in range(2)]
+    procs = [ctx.Process(target=_two_gpu_worker, args=(i, 2, port, fuse, acquire, q)) for i in range(2)]
     for p in procs:
         p.start()
     got = sorted((q.get(timeout=600) for _ in procs), key=lambda g: g["rank"])
