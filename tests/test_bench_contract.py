@@ -56,3 +56,30 @@ def test_reference_arm_other_ranks_exit_quietly():
     out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--config", "1", "--gpus", "2"],
                          capture_output=True, text=True, timeout=300, cwd=ROOT, env=env)
     assert out.returncode == 0 and out.stdout.strip() == ""
+
+
+def test_config_says_which_loop_runs_and_whether_the_workload_is_l2_resident():
+    """bench.py's copy of the library's rule (one cooperative kernel where the stored links take at most a third of the
+    L2; never against an explicit --cg-mode sync; fp64 staggered solves only) and the l2_policy derived from the link
+    bytes.  The GPU arm checks the rule against lqcd_last_cg_path() and overrides `config` if the library chose otherwise."""
+    import argparse
+    import bench
+    from paper_1311_2719_b200 import synth
+    ns = lambda **kw: argparse.Namespace(**dict(dict(precision="f64", recon=18, cg_mode="graph", check_every=8), **kw))
+    want = {1: "persistent", 2: "persistent", 3: "host_loop", 4: "host_loop", 5: "host_loop"}
+    for n, path in want.items():
+        c = bench.config_dict(ns(), synth.config(n), 1)
+        assert c["cg_path"] == path and (c["check_every"] is None) == (path == "persistent")
+        assert ("L2-RESIDENT" in c["l2_policy"]) == (path == "persistent")
+        assert ("larger than L2" in c["l2_policy"]) == (n in (3, 5))
+    assert bench.config_dict(ns(cg_mode="sync"), synth.config(2), 1)["cg_path"] == "host_loop"
+    assert bench.config_dict(ns(precision="mixed"), synth.config(2), 1)["cg_path"] == "host_loop"
+    # what `configs` keeps of a full line
+    line = {"config": {"workload": "w", "l2_policy": "p"}, "cg": {"path": "host_loop", "iters": 5, "true_residual": 1e-11,
+            "us_per_iteration": 2.0}, "steps": 3, "warmup": 3, "ms_per_step": 0.01, "value": 1.0,
+            "dslash": {"us_per_call": 1.0, "GBps": 2.0, "GFLOPs": 3.0}, "roofline": {"frac": 0.5, "kernel": "k"},
+            "e2e": {"ms_per_step": 0.02}, "gpu_launches": 7, "clocks": {"sm_mhz": 1965.0},
+            "variants": {"v": {"time_to_solution_ms": 1.0, "iters": 5, "GBps": 9.0}}}
+    e = bench.config_entry(line)
+    assert e["cg_ms"] == 0.01 and e["iters"] == 5 and e["dslash_frac_of_peak"] == 0.5 and e["e2e_ms"] == 0.02
+    assert e["variants"]["v"]["time_to_solution_ms"] == 1.0 and e["cg_path"] == "host_loop"
